@@ -1,0 +1,304 @@
+"""Pins of the CPU oracle's time step (oracle/mmo_scheme.c) against what the paper and the
+mathematics fix -- invariants, closed forms and the exact Euler Riemann solution; none of them
+re-types the oracle's update loop.
+
+  * a uniform state stays uniform (bitwise), also next to Dirichlet ghosts holding that state;
+  * on a periodic box all moments are conserved to round-off without collisions, and
+    rho, rho u_i, tr U_ij with collisions (Eqs 17-18: C_1 = C_i = C_ii = 0);
+  * x <-> y transpose symmetry of a full 2-D run (one routine, indices swapped);
+  * a y-uniform 2-D run has identical rows;
+  * uniform non-equilibrium gas, constant tau: forward Euler gives
+    U_eq + (U_0 - U_eq)(1 - dt/tau)^n exactly (BGK is linear in U at fixed rho, u, P);
+  * one first-order step equals the textbook finite-volume update assembled from the
+    (separately pinned) pointwise flux / wave-speed / interface-flux functions;
+  * the small-Kn Sod solution approaches the exact Euler Riemann solution (gamma = 3 for the
+    1D1V gas, gamma = 5/3 for the 14-moment gas; values from SURVEY.md section 8(c)).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import mm_workloads as wl
+
+
+def oracle_solver(mmo, prob, nthreads=0, **override):
+    opt = dict(prob["options"]); opt.update(override)
+    s = mmo.Solver(prob["system"], prob["nx"], prob["ny"], extent=prob["extent"],
+                   collision=prob["collision"], bcs=prob["bcs"], nthreads=nthreads, **opt)
+    s.set_state_prim(prob["W0"])
+    return s
+
+
+# ----------------------------------------------------------------------------- uniform
+@pytest.mark.parametrize("bc", ["periodic", "transmissive", "dirichlet"])
+def test_uniform_state_stays_uniform_14(mmo, bc):
+    W = np.array([0.7, 0.4, -0.3, 0.2, 0.8, 0.05, -0.02, 0.6, 0.03, 0.7, 0.05, -0.04, 0.02, 1.9])
+    nx, ny = 9, 7
+    W0 = np.broadcast_to(W[:, None, None], (14, ny, nx)).copy()
+    t = {"periodic": wl.BC_PERIODIC, "transmissive": wl.BC_TRANSMISSIVE}.get(bc)
+    bcs = [dict(type=t)] * 4 if t is not None else [dict(type=wl.BC_DIRICHLET, bands=[], default=W)] * 4
+    s = mmo.Solver(14, nx, ny, extent=(0, 1, 0, 1), bcs=bcs,
+                   collision=dict(model=wl.TAU_NONE))
+    s.set_state_prim(W0)
+    U0 = s.get_state()
+    s.step(5, 0.4)
+    U = s.get_state()
+    for m in range(14):
+        assert np.all(U[m] == U[m, 0, 0])
+        # collisionless + uniform => nothing changes at all
+        assert np.all(U[m] == U0[m])
+
+
+def test_uniform_state_stays_uniform_5(mmo):
+    W = np.array([0.7, 0.4, 0.8, 0.1, 3.2])
+    W0 = np.broadcast_to(W[:, None, None], (5, 1, 11)).copy()
+    s = mmo.Solver(5, 11, 1, bcs=[dict(type=wl.BC_TRANSMISSIVE)] * 4)
+    s.set_state_prim(W0)
+    U0 = s.get_state()
+    s.step(5, 0.5)
+    assert np.array_equal(s.get_state(), U0)
+
+
+# ------------------------------------------------------------------------ conservation
+@pytest.mark.parametrize("limiter,shared,flux", [(wl.LIM_MINMOD, 0, wl.FLUX_HLL),
+                                                 (wl.LIM_VANALBADA, 1, wl.FLUX_RUSANOV)])
+def test_periodic_conservation_14(mmo, limiter, shared, flux):
+    prob = wl.random_smooth14(24, 16, limiter=limiter, shared_limiter=shared, flux=flux)
+    s = oracle_solver(mmo, prob)
+    U0 = s.get_state()
+    s.step(10, 0.4)
+    U1 = s.get_state()
+    assert not np.allclose(U0, U1, rtol=1e-3, atol=0)           # something happened
+    for m in range(14):
+        scale = np.abs(U0[m]).sum()
+        assert abs(U1[m].sum() - U0[m].sum()) <= 2e-14 * scale, m
+    # with collisions: mass, momentum, energy (trace of U_ij)
+    prob = wl.random_smooth14(24, 16, Kn=0.05, limiter=limiter, shared_limiter=shared, flux=flux)
+    s = oracle_solver(mmo, prob)
+    U0 = s.get_state()
+    s.step(10, 0.4)
+    U1 = s.get_state()
+    E0 = U0[4] + U0[7] + U0[9]; E1 = U1[4] + U1[7] + U1[9]
+    for a, b in [(U0[0], U1[0]), (U0[1], U1[1]), (U0[2], U1[2]), (U0[3], U1[3]), (E0, E1)]:
+        assert abs(b.sum() - a.sum()) <= 2e-14 * np.abs(a).sum()
+    # ... and the non-conserved ones do change through the source
+    assert abs(U1[13].sum() - U0[13].sum()) > 1e-8 * np.abs(U0[13]).sum()
+
+
+def test_periodic_conservation_5(mmo):
+    prob = wl.random_smooth5(64)
+    s = oracle_solver(mmo, prob)
+    U0 = s.get_state(); s.step(20, 0.5); U1 = s.get_state()
+    for m in range(5):
+        assert abs(U1[m].sum() - U0[m].sum()) <= 2e-14 * np.abs(U0[m]).sum()
+    prob = wl.random_smooth5(64, Kn=0.05)
+    s = oracle_solver(mmo, prob)
+    U0 = s.get_state(); s.step(20, 0.5); U1 = s.get_state()
+    for m in range(3):
+        assert abs(U1[m].sum() - U0[m].sum()) <= 2e-14 * np.abs(U0[m]).sum()
+    assert abs(U1[4].sum() - U0[4].sum()) > 1e-8 * np.abs(U0[4]).sum()
+
+
+# ---------------------------------------------------------------------------- symmetry
+# x <-> y swap of the 14 primitives / conserved moments (u, P, q components)
+SWAP_XY = [0, 2, 1, 3, 7, 5, 8, 4, 6, 9, 11, 10, 12, 13]
+
+
+def test_transpose_symmetry(mmo):
+    prob = wl.random_smooth14(12, 12, Kn=0.1)
+    sA = oracle_solver(mmo, prob)
+    WT = prob["W0"][SWAP_XY].transpose(0, 2, 1).copy()
+    probT = dict(prob, W0=WT)
+    sB = oracle_solver(mmo, probT)
+    sA.step_fixed_dt(6, 2e-3); sB.step_fixed_dt(6, 2e-3)
+    UA = sA.get_state(); UB = sB.get_state()[SWAP_XY].transpose(0, 2, 1)
+    scale = np.abs(UA).max(axis=(1, 2), keepdims=True)
+    assert np.max(np.abs(UA - UB) / scale) < 1e-13
+
+
+def test_y_uniform_rows_identical(mmo):
+    prob = wl.sod14(64, 4, Kn=0.01)
+    s = oracle_solver(mmo, prob)
+    s.step(20, 0.5)
+    U = s.get_state()
+    for j in range(1, 4):
+        assert np.array_equal(U[:, j], U[:, 0])
+    # z-odd and y-odd moments stay exactly zero
+    for m in (2, 3, 5, 6, 8, 11, 12):
+        assert np.all(U[m] == 0.0)
+
+
+# -------------------------------------------------------------------------- relaxation
+def test_uniform_relaxation_is_geometric(mmo):
+    W = np.array([0.7, 0.4, -0.3, 0.2, 0.8, 0.05, -0.02, 0.6, 0.03, 0.7, 0.05, -0.04, 0.02, 1.9])
+    nx, ny = 5, 4
+    W0 = np.broadcast_to(W[:, None, None], (14, ny, nx)).copy()
+    tau, dt, n = 0.05, 0.004, 25
+    s = mmo.Solver(14, nx, ny, bcs=[dict(type=wl.BC_PERIODIC)] * 4,
+                   collision=dict(model=wl.TAU_CONST, tau=tau))
+    s.set_state_prim(W0)
+    U0 = s.get_state()[:, 0, 0]
+    s.step_fixed_dt(n, dt)
+    Un = s.get_state()[:, 0, 0]
+    # equilibrium: same rho, u, hydrostatic P; Maxwellian moments (L73)
+    P = (W[4] + W[7] + W[9]) / 3
+    Weq = wl.maxwellian(14, W[0], W[1:4], P / W[0])
+    se = mmo.Solver(14, 1, 1, bcs=[dict(type=wl.BC_PERIODIC)] * 4)
+    se.set_state_prim(Weq.reshape(14, 1, 1))
+    Ueq = se.get_state()[:, 0, 0]
+    expect = Ueq + (U0 - Ueq) * (1 - dt / tau) ** n
+    assert np.allclose(Un, expect, rtol=1e-12, atol=1e-13)
+    assert np.abs(U0 - Ueq).max() > 0.05
+
+    W5 = np.array([0.7, 0.4, 0.8, 0.1, 3.2])
+    s = mmo.Solver(5, 4, 1, bcs=[dict(type=wl.BC_PERIODIC)] * 4,
+                   collision=dict(model=wl.TAU_CONST, tau=tau))
+    s.set_state_prim(np.broadcast_to(W5[:, None, None], (5, 1, 4)).copy())
+    U0 = s.get_state()[:, 0, 0]
+    s.step_fixed_dt(n, dt)
+    Un = s.get_state()[:, 0, 0]
+    Ueq = mmo.prim2cons(wl.maxwellian(5, W5[0], W5[1], W5[2] / W5[0]))
+    assert np.allclose(Un, Ueq + (U0 - Ueq) * (1 - dt / tau) ** n, rtol=1e-12, atol=1e-13)
+
+
+# ------------------------------------------------- one first-order step, textbook assembly
+def test_first_order_step_is_textbook_fv_update(mmo):
+    """LIM_NONE => piecewise-constant states, so every interface flux is the (pinned) pointwise
+    numerical flux of the two adjacent cell states; the step is U - dt/dx dF - dt/dy dG + dt C
+    (PAPER.md L250).  Assembled here in numpy with periodic wrap-around by np.roll."""
+    prob = wl.random_smooth14(6, 5, Kn=0.2, limiter=wl.LIM_NONE)
+    s = oracle_solver(mmo, prob)
+    nx, ny = 6, 5
+    dx, dy = 1.0 / nx, (ny / nx) / ny
+    W0 = prob["W0"]
+    U0 = s.get_state()
+    dt = 1.3e-3
+    s.step_fixed_dt(1, dt)
+    U1 = s.get_state()
+
+    def hat(WL, WR, d):
+        FL, FR = mmo.flux14(WL, d, 1e-4), mmo.flux14(WR, d, 1e-4)
+        a, b = mmo.wavespeed14(WL, d, 1e-4), mmo.wavespeed14(WR, d, 1e-4)
+        return mmo.numflux(wl.FLUX_HLL, FL, FR, mmo.prim2cons(WL), mmo.prim2cons(WR), a[0], a[1], b[0], b[1])
+
+    exp = np.empty_like(U0)
+    for j in range(ny):
+        for i in range(nx):
+            Wc = W0[:, j, i]
+            Fe = hat(Wc, W0[:, j, (i + 1) % nx], 0); Fw = hat(W0[:, j, (i - 1) % nx], Wc, 0)
+            Gn = hat(Wc, W0[:, (j + 1) % ny, i], 1); Gs = hat(W0[:, (j - 1) % ny, i], Wc, 1)
+            Ph = (Wc[4] + Wc[7] + Wc[9]) / 3
+            tau = mmo.tau(wl.TAU_KN, 0.0, 0.2, 1.0, 1.0, Wc[0], Ph)
+            exp[:, j, i] = U0[:, j, i] - dt / dx * (Fe - Fw) - dt / dy * (Gn - Gs) + dt * mmo.source14(Wc, tau)
+    scale = np.abs(U0).max(axis=(1, 2), keepdims=True)
+    assert np.max(np.abs(U1 - exp) / scale) < 1e-14
+
+
+def test_second_order_reproduces_linear_data_and_bands(mmo):
+    """MUSCL with either limiter reconstructs linear data exactly (psi = 1), so for a state
+    that is linear in x the interface states are W_i +- slope/2 on both sides, i.e. continuous:
+    the interface flux is then the physical flux of that state (HLL consistency) and the
+    update is a pure central difference of F.  Checked on the density flux: d rho/dt = -d(rho u)/dx."""
+    nx, ny = 16, 3
+    x = (np.arange(nx) + 0.5) / nx
+    W0 = wl.maxwellian(14, np.broadcast_to(1.0 + 0.2 * x, (ny, nx)), (0.5, 0.0, 0.0), 1.0)
+    for lim in (wl.LIM_MINMOD, wl.LIM_VANALBADA):
+        s = mmo.Solver(14, nx, ny, extent=(0, 1, 0, ny / nx), limiter=lim,
+                       bcs=[dict(type=wl.BC_TRANSMISSIVE)] * 2 + [dict(type=wl.BC_PERIODIC)] * 2)
+        s.set_state_prim(W0)
+        U0 = s.get_state(); dt = 1e-3
+        s.step_fixed_dt(1, dt)
+        U1 = s.get_state()
+        drho = (U1[0] - U0[0])[:, 2:-2] / dt
+        assert np.allclose(drho, -0.5 * 0.2, rtol=0, atol=1e-11)
+
+
+def test_dirichlet_bands_select_by_cell_centre(mmo):
+    """Inflow bands (L426): after one step only the first interior column next to a band feels
+    the jet state; rows outside the bands next to the background-valued ghost stay untouched."""
+    prob = wl.crossed_jets(20, Kn=None)
+    s = oracle_solver(mmo, prob)
+    U0 = s.get_state()
+    s.step(1, 0.4)
+    U1 = s.get_state()
+    yc = (np.arange(20) + 0.5) / 20
+    in_band = ((yc >= 0.3) & (yc <= 0.4)) | ((yc >= 0.6) & (yc <= 0.7))
+    changed = np.any(U1[:, :, 0] != U0[:, :, 0], axis=0)
+    assert np.array_equal(changed, in_band)
+    assert np.all(U1[:, :, 2:] == U0[:, :, 2:])
+    # lower jet carries +y momentum, upper jet -y momentum
+    lo = np.where((yc >= 0.3) & (yc <= 0.4))[0]; hi = np.where((yc >= 0.6) & (yc <= 0.7))[0]
+    assert np.all(U1[2, lo, 0] > 0) and np.all(U1[2, hi, 0] < 0)
+
+
+def test_advance_to_and_info(mmo):
+    prob = wl.sod5(100, Kn=0.01)
+    s = oracle_solver(mmo, prob)
+    dt0 = s.cfl_dt(0.5)
+    # equilibrium 5-moment wave speed sqrt(5+sqrt(10)) c at sigma_lim -> dt = cfl dx / that (L434)
+    assert dt0 == pytest.approx(0.5 * 0.01 / 2.856970013872806, rel=5e-3)
+    s.advance_to(0.05, 0.5)
+    inf = s.info()
+    assert inf["t"] == 0.05 and inf["steps"] > 10 and 0 < inf["last_dt"] <= dt0 * 1.0001
+
+
+# ------------------------------------------------------------- Sod -> exact Euler (physics)
+EULER = {  # p*, u*, rho*_L, rho*_R, shock speed, fan head, fan tail
+    3.0: (0.272909467286, 0.60856697289, 0.648643694382, 0.170703638658, 2.27300494425,
+          -1.73205080757, -0.514916861788),
+    5.0 / 3.0: (0.293945187666, 0.841194852169, 0.479689058721, 0.229805749312, 1.84447336705,
+                -1.29099444874, -0.169401312511),
+}
+
+
+def exact_sod_density(x, t, gamma):
+    ps, us, rL, rR, ss, head, tail = EULER[gamma]
+    xi = (x - 0.5) / t
+    aL = math.sqrt(gamma * 1.0 / 1.0)
+    rho = np.where(xi < head, 1.0, 0.0)
+    fan = (xi >= head) & (xi < tail)
+    # left rarefaction: u - a = xi, u + 2a/(g-1) = 2aL/(g-1)
+    a = (2 * aL / (gamma - 1) - xi) * (gamma - 1) / (gamma + 1)
+    rho = np.where(fan, (a / aL) ** (2 / (gamma - 1)), rho)
+    rho = np.where((xi >= tail) & (xi < us), rL, rho)
+    rho = np.where((xi >= us) & (xi < ss), rR, rho)
+    rho = np.where(xi >= ss, 0.125, rho)
+    return rho
+
+
+def test_exact_riemann_table_is_self_consistent():
+    """The tabulated star states satisfy the Rankine-Hugoniot and isentropic relations."""
+    for g, (ps, us, rL, rR, ss, head, tail) in EULER.items():
+        assert rL == pytest.approx(ps ** (1 / g), rel=1e-9)
+        assert 0.125 * ss == pytest.approx(rR * (ss - us), rel=1e-9)            # mass across shock
+        assert ps - 0.1 == pytest.approx(0.125 * ss * us, rel=1e-9)             # momentum
+        assert head == pytest.approx(-math.sqrt(g), rel=1e-9)
+        assert tail == pytest.approx(us - math.sqrt(g * ps / rL), rel=1e-9)
+
+
+def test_sod5_approaches_euler_gamma3(mmo):
+    nx = 400
+    x = (np.arange(nx) + 0.5) / nx
+    ref = exact_sod_density(x, 0.2, 3.0)
+    errs = []
+    for Kn in (0.1, 0.01, 0.001):
+        s = oracle_solver(mmo, wl.sod5(nx, Kn=Kn))
+        s.advance_to(0.2, 0.5)
+        errs.append(np.abs(s.get_state()[0, 0] - ref).mean())
+    assert errs[0] > errs[1] > errs[2]
+    assert errs[2] < 0.02 and errs[0] > 2.0 * errs[2]
+
+
+def test_sod14_approaches_euler_gamma53(mmo):
+    nx = 200
+    x = (np.arange(nx) + 0.5) / nx
+    ref = exact_sod_density(x, 0.2, 5.0 / 3.0)
+    errs = []
+    for Kn in (0.1, 0.01, 0.001):
+        s = oracle_solver(mmo, wl.sod14(nx, 2, Kn=Kn))
+        s.advance_to(0.2, 0.5)
+        U = s.get_state()
+        errs.append(np.abs(U[0, 0] - ref).mean())
+    assert errs[0] > errs[1] > errs[2]
+    assert errs[2] < 0.02 and errs[0] > 2.0 * errs[2]
