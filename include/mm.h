@@ -1,0 +1,126 @@
+/*
+ * mm.h -- C-ABI of the B200 (sm_100a) maximum-entropy moment-method time step.
+ *
+ * One thing is computed: the explicit finite-volume time step of the 5-moment (1-D) and
+ * 14-moment (2-D) maximum-entropy systems with the interpolative closure of
+ * Boccelli, Kaufmann, Magin, McDonald, JCP 2024 (arXiv 2401.15233; "PAPER.md"):
+ *   ghost cells (L426) -> conserved->primitive (L264) -> MUSCL + limiter (L262-266) ->
+ *   closure fluxes (Eqs 12-15, 16, 21-25) + approximate wave speeds (Eqs 28-31, 34-35) ->
+ *   HLL / Rusanov interface flux (L256-258) -> forward-Euler update with the BGK source
+ *   (L250; Eqs 12d-e, 17-18) -> CFL max-reduction for the next dt (L434).
+ * Every step of that path runs in CUDA kernels (paper_2401_15233_b200/csrc/); the host code
+ * behind these calls only validates arguments and launches.  There is NO CPU fallback: without
+ * a CUDA device every compute call returns MM_ECUDA.
+ *
+ * Conventions
+ *   - all functions return MM_OK (0) or a negative mm_status; mm_strerror() names it.
+ *   - pointers are HOST pointers unless the argument list says "device"; `on_device` flags
+ *     say which kind a state buffer is.  The caller owns every buffer it passes; tables in
+ *     mm_bc are copied at mm_create.
+ *   - the library never allocates device memory: the caller hands in `d_workspace`
+ *     (>= mm_workspace_bytes(), 256-byte aligned, e.g. a torch uint8 tensor) and a stream;
+ *     all work is enqueued on that stream, nothing synchronises unless stated.
+ *   - solver objects are independent; one object is not thread-safe.
+ *
+ * Moment order (structure of arrays, fp64), field arrays are [moment][ny][nx], interior cells:
+ *   5-moment   conserved U = (rho, rho u, rho u^2+P, rho u^3+3uP+q, rho u^4+6u^2P+4uq+r)   Eq 12
+ *              primitive W = (rho, u, P, q, r)                                              Eq 11
+ *   14-moment  conserved U = (rho | rho u_x,u_y,u_z | U_xx U_xy U_xz U_yy U_yz U_zz |
+ *                             U_xjj U_yjj U_zjj | U_iijj)                                   Eq 16
+ *              primitive W = (rho | u_x u_y u_z | P_xx P_xy P_xz P_yy P_yz P_zz |
+ *                             q_x q_y q_z | R),  q_i = Q_ijj (L183), R = R_iijj             L264
+ */
+#ifndef MM_H
+#define MM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { MM_OK = 0, MM_EINVAL = -1, MM_EWORKSPACE = -2, MM_ECUDA = -3,
+               MM_ENONFINITE = -4 } mm_status;
+
+enum { MM_SYS5_1D = 5, MM_SYS14_2D = 14 };                       /* section 2.3 / 2.4 */
+enum { MM_TAU_NONE = 0, MM_TAU_CONST = 1, MM_TAU_KN = 2 };
+enum { MM_BC_TRANSMISSIVE = 0, MM_BC_PERIODIC = 1, MM_BC_DIRICHLET = 2 };
+enum { MM_LIM_NONE = 0, MM_LIM_MINMOD = 1, MM_LIM_VANALBADA = 2 };
+enum { MM_FLUX_HLL = 0, MM_FLUX_RUSANOV = 1 };
+#define MM_MAX_BANDS 8
+
+typedef struct mm_solver mm_solver;   /* opaque, host object; freed by mm_destroy */
+
+/* Grid: nx x ny interior cells on [x0,x1] x [y0,y1]; ny = 1 (y0,y1 ignored) for MM_SYS5_1D. */
+typedef struct { int system; int nx, ny; double x0, x1, y0, y1; } mm_grid;
+
+/* BGK relaxation time (L284, L474):
+ *   MM_TAU_NONE  collisionless, source disabled (L432)
+ *   MM_TAU_CONST tau
+ *   MM_TAU_KN    tau(rho,P) = Kn L_ref (rho_ref/rho) / sqrt(8 P / (pi rho)),  P hydrostatic,
+ *                i.e. tau = lambda / v_th with lambda ~ 1/rho and Kn = lambda(rho_ref)/L_ref. */
+typedef struct { int model; double tau, Kn, L_ref, rho_ref; } mm_collision;
+
+/* One side of the domain; mm_create takes 4 of them in the order xlo, xhi, ylo, yhi.
+ *   MM_BC_TRANSMISSIVE zero-gradient copy of the adjacent interior cell (L426)
+ *   MM_BC_PERIODIC     both sides of that direction must be periodic
+ *   MM_BC_DIRICHLET    piecewise-constant PRIMITIVE states along the side (inflow jets, L426):
+ *                      band k holds where the cell-centre coordinate along the side is in
+ *                      [band_lo[k], band_hi[k]]; elsewhere default_W, or zero-gradient when
+ *                      default_W == NULL.  nbands <= MM_MAX_BANDS; band_W is [nbands][nmom]. */
+typedef struct { int type; int nbands; const double *band_lo, *band_hi, *band_W;
+                 const double *default_W; } mm_bc;
+
+typedef struct {
+    double sigma_lim;     /* lower limit of sigma inside closure + wave speeds (L163, L512); 1e-4 */
+    double ws_scale;      /* wave-speed inflation k >= 1 (L409); 1.0 */
+    int limiter;          /* MM_LIM_MINMOD | MM_LIM_VANALBADA (L262) | MM_LIM_NONE (1st order) */
+    int shared_limiter;   /* 1: the most stringent limiter value for all primitives (L266) */
+    int flux;             /* MM_FLUX_HLL | MM_FLUX_RUSANOV (L258) */
+    void *stream;         /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
+} mm_options;
+
+/* Bytes of device workspace mm_create needs for this grid (two padded state copies, boundary
+ * tables, control block).  0 on invalid grid. */
+size_t mm_workspace_bytes(const mm_grid *grid);
+
+/* Build a solver on caller-provided device memory.  d_workspace: DEVICE pointer. */
+int mm_create(mm_solver **out, const mm_grid *grid, const mm_collision *collision,
+              const mm_bc bcs[4], const mm_options *options, void *d_workspace, size_t bytes);
+
+/* Load the interior state (conserved resp. primitive moments, [nmom][ny][nx]), fill the ghost
+ * cells and run the CFL reduction; resets t = 0, steps = 0.  Host buffers are copied with
+ * cudaMemcpyAsync on the solver's stream (pin them for true overlap). */
+int mm_set_state(mm_solver *s, const double *U, int on_device);
+int mm_set_state_prim(mm_solver *s, const double *W, int on_device);
+
+/* n forward-Euler steps (L250), each with dt = cfl / max_cells max(s_x/dx, s_y/dy) from the
+ * cell-centre wave speeds of the current state, ghost cells included (L434).  Asynchronous:
+ * dt, t and the step counter live in device memory, nothing is read back. */
+int mm_step(mm_solver *s, int n, double cfl);
+/* n steps with the given dt (parity mode). */
+int mm_step_fixed_dt(mm_solver *s, int n, double dt);
+/* CFL steps until t == t_end (last step clipped); max_steps <= 0: unlimited.  Synchronises. */
+int mm_advance_to(mm_solver *s, double t_end, double cfl, int max_steps);
+
+/* Copy out the interior state; synchronises the stream. */
+int mm_get_state(mm_solver *s, double *U, int on_device);
+int mm_get_state_prim(mm_solver *s, double *W, int on_device);
+
+/* t, completed steps, last dt, max wave speed of the current state (any pointer may be NULL).
+ * Synchronises.  Returns MM_ENONFINITE if the CFL reduction met rho <= 0, P <= 0 or a
+ * non-finite wave speed; from that point on steps leave the state untouched. */
+int mm_get_info(mm_solver *s, double *t, long long *steps, double *last_dt, double *max_speed);
+/* dt the next mm_step(., cfl) would take.  Synchronises. */
+int mm_cfl_dt(mm_solver *s, double cfl, double *dt);
+
+/* Number of kernel launches enqueued by this solver so far. */
+long long mm_launch_count(const mm_solver *s);
+
+void mm_destroy(mm_solver *s);
+const char *mm_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MM_H */

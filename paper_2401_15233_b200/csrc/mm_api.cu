@@ -1,0 +1,374 @@
+// mm_api.cu -- host side of the C-ABI in include/mm.h: argument checks, workspace carving and
+// kernel launches.  No arithmetic of the method runs here; there is no CPU fallback.
+#include "../../include/mm.h"
+#include "mm_kernels.cuh"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace mm;
+
+namespace {
+
+constexpr int kTX = 32, kTY = 8;        // 14-moment tile (cells per block)
+constexpr int kNT5 = 128;               // 5-moment cells per block
+constexpr int kRateNT = 256;
+
+thread_local char g_cuda_msg[256] = "";
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    int nm, pitch, rows;
+    size_t plane, state_bytes, off_ctrl, off_bc, off_u0, off_u1, total;
+};
+
+bool make_layout(const mm_grid* g, Layout* L)
+{
+    if (!g) return false;
+    if (g->system != MM_SYS5_1D && g->system != MM_SYS14_2D) return false;
+    if (g->nx < 1 || g->ny < 1 || !(g->x1 > g->x0)) return false;
+    if (g->system == MM_SYS5_1D && g->ny != 1) return false;
+    if (g->system == MM_SYS14_2D && !(g->y1 > g->y0)) return false;
+    L->nm = g->system;
+    L->pitch = (int)align_up((size_t)g->nx + 4, 16);
+    L->rows = g->ny + 4;
+    L->plane = (size_t)L->pitch * L->rows;
+    L->state_bytes = align_up(L->plane * L->nm * sizeof(double), 256);
+    L->off_ctrl = 0;
+    L->off_bc = align_up(sizeof(Ctrl), 256);
+    L->off_u0 = L->off_bc + align_up(sizeof(BcTable), 256);
+    L->off_u1 = L->off_u0 + L->state_bytes;
+    L->total = L->off_u1 + L->state_bytes;
+    return true;
+}
+
+}  // namespace
+
+struct mm_solver {
+    mm_grid grid;
+    Layout L;
+    Params p;
+    cudaStream_t stream;
+    char* ws;
+    Ctrl* ctrl;
+    BcTable* bc;
+    double* U[2];
+    int cur;            // buffer holding the current state
+    int slot;           // accumulator slot holding the current state's CFL reduction
+    int has_state;
+    long long launches;
+    size_t smem14;
+};
+
+namespace {
+
+int cuda_fail(cudaError_t e, const char* what)
+{
+    snprintf(g_cuda_msg, sizeof g_cuda_msg, "CUDA error in %s: %s", what, cudaGetErrorString(e));
+    return MM_ECUDA;
+}
+#define MM_CUDA(call)                                                        \
+    do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+#define MM_LAUNCHED(s, what)                                                 \
+    do { (s)->launches++; cudaError_t e_ = cudaGetLastError();               \
+         if (e_ != cudaSuccess) return cuda_fail(e_, what); } while (0)
+
+template <int NM>
+int launch_ghost(mm_solver* s, const StepCtl& sc, int finalize)
+{
+    const int n = 4 * s->p.ny + (NM == 5 ? 0 : 4 * s->p.nx);
+    const int nt = 128, nb = (n + nt - 1) / nt;
+    k_ghost<NM><<<nb, nt, 0, s->stream>>>(s->p, s->U[s->cur], s->bc, s->ctrl, s->slot, sc, finalize);
+    MM_LAUNCHED(s, "k_ghost");
+    return MM_OK;
+}
+
+int launch_step(mm_solver* s, const StepCtl& sc)
+{
+    int rc;
+    if (s->L.nm == 5) {
+        if ((rc = launch_ghost<5>(s, sc, 1))) return rc;
+        const int nb = (s->p.nx + kNT5 - 1) / kNT5;
+        k_step5<kNT5><<<nb, kNT5, 0, s->stream>>>(s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1);
+        MM_LAUNCHED(s, "k_step5");
+    } else {
+        if ((rc = launch_ghost<14>(s, sc, 1))) return rc;
+        dim3 grid((s->p.nx + kTX - 1) / kTX, (s->p.ny + kTY - 1) / kTY);
+        k_step14<kTX, kTY><<<grid, kTX * kTY, s->smem14, s->stream>>>(
+            s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1);
+        MM_LAUNCHED(s, "k_step14");
+    }
+    s->cur ^= 1;
+    s->slot ^= 1;
+    return MM_OK;
+}
+
+int read_ctrl(mm_solver* s, Ctrl* h)
+{
+    MM_CUDA(cudaMemcpyAsync(h, s->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, s->stream));
+    MM_CUDA(cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
+
+double bits2d(unsigned long long b) { double d; memcpy(&d, &b, 8); return d; }
+
+template <int NM>
+int set_state_impl(mm_solver* s, const double* src, int on_device, bool prim)
+{
+    const size_t nbytes = (size_t)NM * s->p.nx * s->p.ny * sizeof(double);
+    const double* dsrc = src;
+    if (!on_device) {   // stage through the idle state copy
+        MM_CUDA(cudaMemcpyAsync(s->U[s->cur ^ 1], src, nbytes, cudaMemcpyHostToDevice, s->stream));
+        dsrc = s->U[s->cur ^ 1];
+    }
+    dim3 grid((s->p.nx + 127) / 128, s->p.ny);
+    if (prim) k_pack<NM, true><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur]);
+    else k_pack<NM, false><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur]);
+    MM_LAUNCHED(s, "k_pack");
+    // reset the clock and the accumulators (keeps the constant ghost part)
+    MM_CUDA(cudaMemsetAsync(s->ctrl, 0, offsetof(Ctrl, ghost_rate), s->stream));
+    MM_CUDA(cudaMemsetAsync(&s->ctrl->steps, 0, sizeof(Ctrl) - offsetof(Ctrl, steps), s->stream));
+    s->slot = 0;
+    StepCtl none = {0, 0.0, -1.0};
+    int rc = launch_ghost<NM>(s, none, 0);
+    if (rc) return rc;
+    const long long n = (long long)s->p.nx * s->p.ny;
+    int nb = (int)((n + kRateNT - 1) / kRateNT);
+    if (nb > 148 * 8) nb = 148 * 8;
+    k_rate<NM, kRateNT><<<nb, kRateNT, 0, s->stream>>>(s->p, s->U[s->cur], s->ctrl, 0);
+    MM_LAUNCHED(s, "k_rate");
+    s->has_state = 1;
+    return MM_OK;
+}
+
+template <int NM>
+int get_state_impl(mm_solver* s, double* dst, int on_device, bool prim)
+{
+    const size_t nbytes = (size_t)NM * s->p.nx * s->p.ny * sizeof(double);
+    double* ddst = on_device ? dst : s->U[s->cur ^ 1];
+    dim3 grid((s->p.nx + 127) / 128, s->p.ny);
+    if (prim) k_unpack<NM, true><<<grid, 128, 0, s->stream>>>(s->p, s->U[s->cur], ddst);
+    else k_unpack<NM, false><<<grid, 128, 0, s->stream>>>(s->p, s->U[s->cur], ddst);
+    MM_LAUNCHED(s, "k_unpack");
+    if (!on_device)
+        MM_CUDA(cudaMemcpyAsync(dst, ddst, nbytes, cudaMemcpyDeviceToHost, s->stream));
+    MM_CUDA(cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t mm_workspace_bytes(const mm_grid* grid)
+{
+    Layout L;
+    return make_layout(grid, &L) ? L.total : 0;
+}
+
+int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, const mm_bc bcs[4],
+              const mm_options* opt, void* d_workspace, size_t bytes)
+{
+    if (!out || !grid || !col || !bcs || !opt) return MM_EINVAL;
+    Layout L;
+    if (!make_layout(grid, &L)) return MM_EINVAL;
+    if (!(opt->sigma_lim > 0.0) || !(opt->ws_scale > 0.0)) return MM_EINVAL;
+    if (opt->limiter < 0 || opt->limiter > 2 || opt->flux < 0 || opt->flux > 1) return MM_EINVAL;
+    if (col->model < 0 || col->model > 2) return MM_EINVAL;
+    if (col->model == MM_TAU_CONST && !(col->tau > 0.0)) return MM_EINVAL;
+    if (col->model == MM_TAU_KN && !(col->Kn > 0.0 && col->L_ref > 0.0 && col->rho_ref > 0.0)) return MM_EINVAL;
+    const int ndim = grid->system == MM_SYS5_1D ? 1 : 2;
+    for (int b = 0; b < 2 * ndim; ++b) {
+        if (bcs[b].type < 0 || bcs[b].type > 2) return MM_EINVAL;
+        if (bcs[b].type == MM_BC_DIRICHLET) {
+            if (bcs[b].nbands < 0 || bcs[b].nbands > MM_MAX_BANDS) return MM_EINVAL;
+            if (bcs[b].nbands > 0 && (!bcs[b].band_lo || !bcs[b].band_hi || !bcs[b].band_W)) return MM_EINVAL;
+        }
+    }
+    for (int d = 0; d < ndim; ++d)
+        if ((bcs[2 * d].type == MM_BC_PERIODIC) != (bcs[2 * d + 1].type == MM_BC_PERIODIC)) return MM_EINVAL;
+    if (!d_workspace || bytes < L.total || ((size_t)d_workspace & 255)) return MM_EWORKSPACE;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return cuda_fail(cudaErrorNoDevice, "mm_create (no CUDA device: this library has no CPU path)");
+
+    mm_solver* s = new (std::nothrow) mm_solver();
+    if (!s) return MM_EINVAL;
+    s->grid = *grid; s->L = L;
+    s->stream = (cudaStream_t)opt->stream;
+    s->ws = (char*)d_workspace;
+    s->ctrl = (Ctrl*)(s->ws + L.off_ctrl);
+    s->bc = (BcTable*)(s->ws + L.off_bc);
+    s->U[0] = (double*)(s->ws + L.off_u0);
+    s->U[1] = (double*)(s->ws + L.off_u1);
+    Params& p = s->p;
+    p.sigma_lim = opt->sigma_lim; p.ws_scale = opt->ws_scale;
+    p.dx = (grid->x1 - grid->x0) / grid->nx;
+    p.dy = ndim == 2 ? (grid->y1 - grid->y0) / grid->ny : 1.0;
+    p.x0 = grid->x0; p.y0 = ndim == 2 ? grid->y0 : 0.0;
+    p.inv_tau_coef = col->model == MM_TAU_KN ? 1.0 / (col->Kn * col->L_ref * col->rho_ref) : 0.0;
+    p.inv_tau_const = col->model == MM_TAU_CONST ? 1.0 / col->tau : 0.0;
+    p.tau_model = col->model; p.limiter = opt->limiter;
+    p.shared_limiter = opt->shared_limiter ? 1 : 0; p.flux = opt->flux;
+    p.nx = grid->nx; p.ny = grid->ny; p.pitch = L.pitch; p.rows = L.rows;
+
+    // boundary tables: copy, and mark which entries some ghost cell actually takes
+    BcTable* hb = new (std::nothrow) BcTable();
+    if (!hb) { delete s; return MM_EINVAL; }
+    memset(hb, 0, sizeof *hb);
+    const int nm = L.nm;
+    for (int b = 0; b < 2 * ndim; ++b) {
+        BcSide& sd = hb->side[b];
+        sd.type = bcs[b].type;
+        if (sd.type != MM_BC_DIRICHLET) continue;
+        sd.nbands = bcs[b].nbands;
+        sd.has_default = bcs[b].default_W ? 1 : 0;
+        for (int k = 0; k < sd.nbands; ++k) {
+            sd.lo[k] = bcs[b].band_lo[k]; sd.hi[k] = bcs[b].band_hi[k];
+            memcpy(sd.W[k], bcs[b].band_W + (size_t)k * nm, nm * sizeof(double));
+        }
+        if (sd.has_default) memcpy(sd.W[sd.nbands], bcs[b].default_W, nm * sizeof(double));
+        const int n = b < 2 ? grid->ny : grid->nx;
+        for (int pos = 0; pos < n; ++pos) {
+            const double coord = b < 2 ? p.y0 + ((double)pos + 0.5) * p.dy : p.x0 + ((double)pos + 0.5) * p.dx;
+            int k = sd.has_default ? sd.nbands : -1;
+            for (int q = sd.nbands - 1; q >= 0; --q)
+                if (coord >= sd.lo[q] && coord <= sd.hi[q]) k = q;
+            if (k >= 0) sd.used |= 1u << k;
+        }
+    }
+    cudaError_t e = cudaMemsetAsync(s->ws, 0, L.total, s->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s->bc, hb, sizeof(BcTable), cudaMemcpyHostToDevice, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);   // hb is pageable: copy done before delete
+    delete hb;
+    if (e != cudaSuccess) { delete s; return cuda_fail(e, "mm_create workspace init"); }
+
+    s->smem14 = (size_t)14 * ((kTY + 4) * (kTX + 4) + kTY * (kTX + 1) + (kTY + 1) * kTX) * sizeof(double);
+    if (nm == 14) {
+        e = cudaFuncSetAttribute(k_step14<kTX, kTY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->smem14);
+        if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaFuncSetAttribute(k_step14)"); }
+        k_bc_table<14><<<4, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 4);
+    } else {
+        k_bc_table<5><<<2, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 2);
+    }
+    s->launches++;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { delete s; return cuda_fail(e, "k_bc_table"); }
+    *out = s;
+    return MM_OK;
+}
+
+int mm_set_state(mm_solver* s, const double* U, int on_device)
+{
+    if (!s || !U) return MM_EINVAL;
+    return s->L.nm == 5 ? set_state_impl<5>(s, U, on_device, false) : set_state_impl<14>(s, U, on_device, false);
+}
+
+int mm_set_state_prim(mm_solver* s, const double* W, int on_device)
+{
+    if (!s || !W) return MM_EINVAL;
+    return s->L.nm == 5 ? set_state_impl<5>(s, W, on_device, true) : set_state_impl<14>(s, W, on_device, true);
+}
+
+int mm_get_state(mm_solver* s, double* U, int on_device)
+{
+    if (!s || !U || !s->has_state) return MM_EINVAL;
+    return s->L.nm == 5 ? get_state_impl<5>(s, U, on_device, false) : get_state_impl<14>(s, U, on_device, false);
+}
+
+int mm_get_state_prim(mm_solver* s, double* W, int on_device)
+{
+    if (!s || !W || !s->has_state) return MM_EINVAL;
+    return s->L.nm == 5 ? get_state_impl<5>(s, W, on_device, true) : get_state_impl<14>(s, W, on_device, true);
+}
+
+int mm_step(mm_solver* s, int n, double cfl)
+{
+    if (!s || n < 0 || !(cfl > 0.0) || !s->has_state) return MM_EINVAL;
+    StepCtl sc = {1, cfl, -1.0};
+    for (int k = 0; k < n; ++k) {
+        int rc = launch_step(s, sc);
+        if (rc) return rc;
+    }
+    return MM_OK;
+}
+
+int mm_step_fixed_dt(mm_solver* s, int n, double dt)
+{
+    if (!s || n < 0 || !(dt > 0.0) || !s->has_state) return MM_EINVAL;
+    StepCtl sc = {0, dt, -1.0};
+    for (int k = 0; k < n; ++k) {
+        int rc = launch_step(s, sc);
+        if (rc) return rc;
+    }
+    return MM_OK;
+}
+
+int mm_advance_to(mm_solver* s, double t_end, double cfl, int max_steps)
+{
+    if (!s || !(cfl > 0.0) || !(t_end >= 0.0) || !s->has_state) return MM_EINVAL;
+    Ctrl h;
+    int rc = read_ctrl(s, &h);
+    if (rc) return rc;
+    const long long first = h.steps;
+    StepCtl sc = {1, cfl, t_end};
+    while (h.t < t_end && !h.failed) {
+        long long left = max_steps > 0 ? max_steps - (h.steps - first) : (1ll << 40);
+        if (left <= 0) break;
+        // enqueue about as many steps as the current dt suggests; steps past t_end only copy
+        double rate = fmax(bits2d(h.rate_bits[s->slot]), h.ghost_rate);
+        double est = rate > 0.0 ? (t_end - h.t) * rate / cfl : 1.0;
+        long long batch = est < 1.0 ? 1 : (est > 256.0 ? 256 : (long long)est + 1);
+        if (batch > left) batch = left;
+        for (long long k = 0; k < batch; ++k)
+            if ((rc = launch_step(s, sc))) return rc;
+        if ((rc = read_ctrl(s, &h))) return rc;
+    }
+    return h.failed ? MM_ENONFINITE : MM_OK;
+}
+
+int mm_get_info(mm_solver* s, double* t, long long* steps, double* last_dt, double* max_speed)
+{
+    if (!s) return MM_EINVAL;
+    Ctrl h;
+    int rc = read_ctrl(s, &h);
+    if (rc) return rc;
+    if (t) *t = h.t;
+    if (steps) *steps = h.steps;
+    if (last_dt) *last_dt = h.last_dt;
+    if (max_speed) *max_speed = fmax(bits2d(h.speed_bits[s->slot]), h.ghost_speed);
+    return (h.failed || h.bc_bad || h.bad[s->slot]) ? MM_ENONFINITE : MM_OK;
+}
+
+int mm_cfl_dt(mm_solver* s, double cfl, double* dt)
+{
+    if (!s || !dt || !(cfl > 0.0) || !s->has_state) return MM_EINVAL;
+    Ctrl h;
+    int rc = read_ctrl(s, &h);
+    if (rc) return rc;
+    double rate = fmax(bits2d(h.rate_bits[s->slot]), h.ghost_rate);
+    if (h.failed || h.bc_bad || h.bad[s->slot] || !(rate > 0.0)) return MM_ENONFINITE;
+    *dt = cfl / rate;
+    return MM_OK;
+}
+
+long long mm_launch_count(const mm_solver* s) { return s ? s->launches : 0; }
+
+void mm_destroy(mm_solver* s) { delete s; }
+
+const char* mm_strerror(int status)
+{
+    switch (status) {
+    case MM_OK: return "ok";
+    case MM_EINVAL: return "invalid argument";
+    case MM_EWORKSPACE: return "workspace missing, too small or not 256-byte aligned";
+    case MM_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
+    case MM_ENONFINITE: return "CFL reduction met rho <= 0, P <= 0 or a non-finite wave speed";
+    default: return "unknown status";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,451 @@
+// mm_kernels.cuh -- CUDA kernels of the moment-method time step (sm_100a, fp64, SoA).
+//
+// Data layout: each state copy is NM planes of `rows` x `pitch` doubles,
+// rows = ny + 4, pitch = roundup(nx + 4, 16); interior cell (i, j) sits at
+// plane[(j + 2) * pitch + (i + 2)], two ghost layers on every side (corner ghosts are never
+// read).  Two copies ping-pong; a control block in device memory carries t, dt, the step
+// counter and the CFL max-reduction accumulators, so a sequence of steps needs no host sync.
+#pragma once
+#include "mm_physics.cuh"
+
+namespace mm {
+
+constexpr int kMaxBands = 8;
+
+// Control block (device memory).  rate = max_cells max(s_x/dx, s_y/dy), speed = max_cells s_d.
+struct Ctrl {
+    double t, dt, last_dt;
+    unsigned long long rate_bits[2], speed_bits[2];   // max-reduced as ordered bit patterns (>= 0)
+    double ghost_rate, ghost_speed;                   // constant part from Dirichlet ghost states
+    long long bc_bad;                                 // a Dirichlet state has rho <= 0 or P <= 0
+    long long steps;
+    int bad[2];                                       // reduction saw rho<=0, P<=0 or non-finite
+    int failed;                                       // sticky: stepping stopped (MM_ENONFINITE)
+    int skip;                                         // this step leaves the state untouched
+};
+
+// Boundary tables (device memory): conserved ghost states of the Dirichlet sides.
+struct BcSide {
+    int type, nbands, has_default;
+    unsigned used;                                    // bit k: table entry k is selected by a ghost cell
+    double lo[kMaxBands], hi[kMaxBands];
+    double W[kMaxBands + 1][14];                      // primitive band states, [nbands] = default
+    double U[kMaxBands + 1][14];                      // conserved, filled by k_bc_table
+};
+struct BcTable { BcSide side[4]; };
+
+__device__ __forceinline__ void atomic_max_pos(unsigned long long* a, double v)
+{
+    atomicMax(a, (unsigned long long)__double_as_longlong(v));
+}
+
+// block-wide max of two non-negative values and OR of a flag, then one atomic per block
+template <int NT>
+__device__ __forceinline__ void block_reduce_rate(double rate, double speed, int bad, Ctrl* ctrl,
+                                                  int slot)
+{
+    __shared__ double s_rate[NT / 32], s_speed[NT / 32];
+    __shared__ int s_bad[NT / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+        speed = fmax(speed, __shfl_xor_sync(0xffffffffu, speed, o));
+        bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) { s_rate[w] = rate; s_speed[w] = speed; s_bad[w] = bad; }
+    __syncthreads();
+    if (w == 0) {
+        rate = l < NT / 32 ? s_rate[l] : 0.0;
+        speed = l < NT / 32 ? s_speed[l] : 0.0;
+        bad = l < NT / 32 ? s_bad[l] : 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+            speed = fmax(speed, __shfl_xor_sync(0xffffffffu, speed, o));
+            bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+        }
+        if (l == 0) {
+            atomic_max_pos(&ctrl->rate_bits[slot], rate);
+            atomic_max_pos(&ctrl->speed_bits[slot], speed);
+            if (bad) atomicOr(&ctrl->bad[slot], 1);
+        }
+    }
+}
+
+// rate / speed / validity of one cell from its conserved moments
+template <int NM>
+__device__ __forceinline__ void cell_rate(const Params& p, const double (&U)[NM], double& rate,
+                                          double& speed, int& bad)
+{
+    double W[NM];
+    bool ok;
+    if constexpr (NM == 5) {
+        cons2prim5(U, W);
+        double sx;
+        ok = cell_speed5(p, W, sx);
+        rate = sx / p.dx; speed = sx;
+    } else {
+        cons2prim14(U, W);
+        double sx, sy;
+        ok = cell_speeds14(p, W, sx, sy);
+        rate = fmax(sx / p.dx, sy / p.dy); speed = fmax(sx, sy);
+    }
+    // finite test: NaN or Inf fail (x - x != 0)
+    if (!ok || !(rate - rate == 0.0)) { bad = 1; rate = 0.0; speed = 0.0; }
+}
+
+// ---------------------------------------------------------------- state in / out kernels
+// interior [NM][ny][nx] (conserved, or primitive when PRIM) -> padded conserved planes
+template <int NM, bool PRIM>
+__global__ void k_pack(Params p, const double* __restrict__ src, double* __restrict__ dst)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= p.nx) return;
+    const size_t plane = (size_t)p.rows * p.pitch, n = (size_t)p.nx * p.ny;
+    double a[NM], b[NM];
+#pragma unroll
+    for (int m = 0; m < NM; ++m) a[m] = src[m * n + (size_t)j * p.nx + i];
+    if constexpr (PRIM) {
+        if constexpr (NM == 5) prim2cons5(a, b); else prim2cons14(a, b);
+    } else {
+#pragma unroll
+        for (int m = 0; m < NM; ++m) b[m] = a[m];
+    }
+#pragma unroll
+    for (int m = 0; m < NM; ++m) dst[m * plane + (size_t)(j + 2) * p.pitch + i + 2] = b[m];
+}
+
+template <int NM, bool PRIM>
+__global__ void k_unpack(Params p, const double* __restrict__ src, double* __restrict__ dst)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= p.nx) return;
+    const size_t plane = (size_t)p.rows * p.pitch, n = (size_t)p.nx * p.ny;
+    double a[NM], b[NM];
+#pragma unroll
+    for (int m = 0; m < NM; ++m) a[m] = src[m * plane + (size_t)(j + 2) * p.pitch + i + 2];
+    if constexpr (PRIM) {
+        if constexpr (NM == 5) cons2prim5(a, b); else cons2prim14(a, b);
+    } else {
+#pragma unroll
+        for (int m = 0; m < NM; ++m) b[m] = a[m];
+    }
+#pragma unroll
+    for (int m = 0; m < NM; ++m) dst[m * n + (size_t)j * p.nx + i] = b[m];
+}
+
+// Dirichlet tables: primitive -> conserved, and the constant ghost contribution to the CFL max
+// (ghost cells are part of the maximum, R13).  One thread per (side, state).
+template <int NM>
+__global__ void k_bc_table(Params p, BcTable* tab, Ctrl* ctrl, int nsides)
+{
+    const int side = blockIdx.x, k = threadIdx.x;
+    if (side >= nsides) return;
+    BcSide& b = tab->side[side];
+    if (b.type != 2) return;
+    const bool is_default = (k == b.nbands);
+    if (k > b.nbands || (is_default && !b.has_default) || !((b.used >> k) & 1u)) return;
+    double W[NM], U[NM];
+#pragma unroll
+    for (int m = 0; m < NM; ++m) W[m] = b.W[k][m];
+    if constexpr (NM == 5) prim2cons5(W, U); else prim2cons14(W, U);
+#pragma unroll
+    for (int m = 0; m < NM; ++m) b.U[k][m] = U[m];
+    double rate, speed; int bad = 0;
+    cell_rate<NM>(p, U, rate, speed, bad);
+    // only entries that some ghost cell actually takes (b.used, set at mm_create) count
+    atomic_max_pos(reinterpret_cast<unsigned long long*>(&ctrl->ghost_rate), rate);
+    atomic_max_pos(reinterpret_cast<unsigned long long*>(&ctrl->ghost_speed), speed);
+    if (bad) ctrl->bc_bad = 1;
+}
+
+// ------------------------------------------------------------------- ghost cells (L426)
+// How a step chooses its dt.
+struct StepCtl {
+    int mode;          // 0: dt = value (fixed), 1: dt = value (= CFL number) / rate
+    double value;
+    double t_end;      // < 0: none; else the step is clipped to land on t_end, later steps skip
+};
+
+// One thread per ghost cell: side-major index over (side, position along the side, layer).
+// Thread 0 also closes the CFL reduction of the state that is about to be stepped:
+// dt = cfl / max(rate, ghost_rate) (L434), advances t and the step counter, and clears the
+// accumulator slot the step kernel will max-reduce the NEXT state into.
+template <int NM>
+__global__ void k_ghost(Params p, double* __restrict__ U, const BcTable* __restrict__ tab,
+                        Ctrl* ctrl, int slot, StepCtl sc, int finalize)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (finalize && tid == 0) {
+        const int bad = ctrl->bad[slot] | ctrl->failed | (int)ctrl->bc_bad;
+        double rate = fmax(__longlong_as_double((long long)ctrl->rate_bits[slot]), ctrl->ghost_rate);
+        double dt = sc.mode == 1 ? sc.value / rate : sc.value;
+        int skip = 0;
+        if (bad || (sc.mode == 1 && !(rate > 0.0))) { ctrl->failed = 1; skip = 1; }
+        double t = ctrl->t, tn = t + dt;
+        if (sc.t_end >= 0.0 && !skip) {
+            if (t >= sc.t_end) skip = 1;
+            else if (tn >= sc.t_end) { dt = sc.t_end - t; tn = sc.t_end; }
+        }
+        if (skip) dt = 0.0;
+        else { ctrl->t = tn; ctrl->steps += 1; ctrl->last_dt = dt; }
+        ctrl->dt = dt;
+        ctrl->skip = skip;
+        // a skipped step carries the state over unchanged, and its reduction with it
+        ctrl->rate_bits[slot ^ 1] = skip ? ctrl->rate_bits[slot] : 0ull;
+        ctrl->speed_bits[slot ^ 1] = skip ? ctrl->speed_bits[slot] : 0ull;
+        ctrl->bad[slot ^ 1] = skip ? ctrl->bad[slot] : 0;
+    }
+    const int nx = p.nx, ny = p.ny;
+    const int nxs = 2 * ny;                     // ghost cells per x side
+    const int nys = (NM == 5) ? 0 : 2 * nx;     // per y side (1-D system has none)
+    if (tid >= 2 * nxs + 2 * nys) return;
+    int side, r;
+    if (tid < 2 * nxs) { side = tid / nxs; r = tid % nxs; }
+    else { const int d = nys > 0 ? nys : 1; side = 2 + (tid - 2 * nxs) / d; r = (tid - 2 * nxs) % d; }
+    const int g = (r & 1) + 1, pos = r >> 1;    // layer 1..2, index along the side
+    const BcSide& b = tab->side[side];
+    int gi, gj, si, sj;                          // ghost cell, source cell (interior coords)
+    double coord;
+    if (side < 2) {
+        gj = sj = pos;
+        coord = __dadd_rn(p.y0, __dmul_rn((double)pos + 0.5, p.dy));
+        if (side == 0) { gi = -g; si = b.type == 1 ? ((nx - g) % nx + nx) % nx : 0; }
+        else { gi = nx - 1 + g; si = b.type == 1 ? (g - 1) % nx : nx - 1; }
+    } else {
+        gi = si = pos;
+        coord = __dadd_rn(p.x0, __dmul_rn((double)pos + 0.5, p.dx));
+        if (side == 2) { gj = -g; sj = b.type == 1 ? ((ny - g) % ny + ny) % ny : 0; }
+        else { gj = ny - 1 + g; sj = b.type == 1 ? (g - 1) % ny : ny - 1; }
+    }
+    const size_t plane = (size_t)p.rows * p.pitch;
+    const size_t gidx = (size_t)(gj + 2) * p.pitch + gi + 2, sidx = (size_t)(sj + 2) * p.pitch + si + 2;
+    const double* fixed = nullptr;
+    if (b.type == 2) {
+        int k = b.has_default ? b.nbands : -1;
+        for (int q = b.nbands - 1; q >= 0; --q)          // first matching band wins
+            if (coord >= b.lo[q] && coord <= b.hi[q]) k = q;
+        if (k >= 0) fixed = b.U[k];
+    }
+#pragma unroll
+    for (int m = 0; m < NM; ++m) U[m * plane + gidx] = fixed ? fixed[m] : U[m * plane + sidx];
+}
+
+// Standalone CFL reduction over the interior (used after mm_set_state).
+template <int NM, int NT>
+__global__ void __launch_bounds__(NT) k_rate(Params p, const double* __restrict__ U, Ctrl* ctrl,
+                                             int slot)
+{
+    const size_t plane = (size_t)p.rows * p.pitch;
+    double rate = 0.0, speed = 0.0;
+    int bad = 0;
+    const long long n = (long long)p.nx * p.ny;
+    for (long long c = (long long)blockIdx.x * NT + threadIdx.x; c < n; c += (long long)gridDim.x * NT) {
+        const int i = (int)(c % p.nx), j = (int)(c / p.nx);
+        double u[NM];
+#pragma unroll
+        for (int m = 0; m < NM; ++m) u[m] = U[m * plane + (size_t)(j + 2) * p.pitch + i + 2];
+        double r, s;
+        cell_rate<NM>(p, u, r, s, bad);
+        rate = fmax(rate, r); speed = fmax(speed, s);
+    }
+    block_reduce_rate<NT>(rate, speed, bad, ctrl, slot);
+}
+
+// ------------------------------------------------------------------ the fused time step
+// Interface flux between cell a (low side) and cell b (high side) along one direction, from the
+// primitives staged in shared memory.  `w` points at cell b of moment plane 0, `cs` is the cell
+// stride along the direction, `ms` the plane stride.  MUSCL on primitives (L262-264): face
+// states W_a + slope_a/2 and W_b - slope_b/2; closure flux, conserved state and wave speeds of
+// both (eval_face*), then HLL / Rusanov.  For the y direction (SWAP) the state is index-swapped
+// on load and the flux swapped back on return (L414).
+template <int NM, bool SWAP>
+__device__ __forceinline__ void interface_flux(const Params& p, const double* __restrict__ w,
+                                               int cs, int ms, double (&Fh)[NM])
+{
+    double WL[NM], WR[NM];
+    if (p.limiter != 0 && p.shared_limiter) {
+        double Wam[NM], Wa[NM], Wb[NM], Wbp[NM], ha[NM], hb[NM];
+#pragma unroll
+        for (int k = 0; k < NM; ++k) {
+            const double* q = w + (SWAP ? swap_xy(k) : k) * ms;
+            Wam[k] = q[-2 * cs]; Wa[k] = q[-cs]; Wb[k] = q[0]; Wbp[k] = q[cs];
+        }
+        half_slopes<NM>(p, Wam, Wa, Wb, ha);
+        half_slopes<NM>(p, Wa, Wb, Wbp, hb);
+#pragma unroll
+        for (int k = 0; k < NM; ++k) { WL[k] = Wa[k] + ha[k]; WR[k] = Wb[k] - hb[k]; }
+    } else {
+#pragma unroll
+        for (int k = 0; k < NM; ++k) {
+            const double* q = w + (SWAP ? swap_xy(k) : k) * ms;
+            const double am = q[-2 * cs], a = q[-cs], b = q[0], bp = q[cs];
+            double ha = 0.0, hb = 0.0;
+            if (p.limiter != 0) {
+                const double d = b - a;
+                ha = 0.5 * limited_slope(p.limiter, a - am, d);
+                hb = 0.5 * limited_slope(p.limiter, d, bp - b);
+            }
+            WL[k] = a + ha; WR[k] = b - hb;
+        }
+    }
+    double FL[NM], UL[NM], FR[NM], UR[NM], lminL, lmaxL, lminR, lmaxR;
+    if constexpr (NM == 5) {
+        eval_face5(p, WL, FL, UL, lminL, lmaxL);
+        eval_face5(p, WR, FR, UR, lminR, lmaxR);
+    } else {
+        eval_face14(p, WL, FL, UL, lminL, lmaxL);
+        eval_face14(p, WR, FR, UR, lminR, lmaxR);
+    }
+    numflux<NM>(p.flux, FL, FR, UL, UR, lminL, lmaxL, lminR, lmaxR, Fh);
+}
+
+// 14-moment 2-D step.  One block = one TX x TY tile of cells:
+//   1. stage the tile + 2-cell halo of the conserved moments in shared memory and convert to
+//      primitives in place (a2);
+//   2. x pass: the (TX+1) x TY x-interfaces of the tile -> Fx (a3-a7);
+//   3. y pass: the TX x (TY+1) y-interfaces -> Fy;
+//   4. one thread per cell: U^{n+1} = U^n - dt/dx dFx - dt/dy dFy + dt C(W^n) (a8), store, then
+//      the wave speeds of the NEW cell state feed the CFL max-reduction for the next dt (a9).
+template <int TX, int TY>
+__global__ void __launch_bounds__(TX * TY)
+k_step14(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl, int slot_next)
+{
+    constexpr int NM = 14, NT = TX * TY, TXH = TX + 4, TYH = TY + 4;
+    constexpr int PW = TYH * TXH, PFX = TY * (TX + 1), PFY = (TY + 1) * TX;
+    extern __shared__ double smem[];
+    double* Ws = smem;                 // [14][TYH][TXH]
+    double* Fx = Ws + NM * PW;         // [14][TY][TX+1]
+    double* Fy = Fx + NM * PFX;        // [14][TY+1][TX]
+    const int tid = threadIdx.x;
+    const int gx0 = blockIdx.x * TX, gy0 = blockIdx.y * TY;
+    const size_t plane = (size_t)p.rows * p.pitch;
+    const double dt = ctrl->dt;
+    const int ci = tid % TX, cj = tid / TX;
+    const bool cell_ok = gx0 + ci < p.nx && gy0 + cj < p.ny;
+    const size_t cidx = (size_t)(gy0 + cj + 2) * p.pitch + gx0 + ci + 2;
+
+    if (ctrl->skip) {                  // failed / past t_end: carry the state over unchanged
+        if (cell_ok)
+#pragma unroll
+            for (int m = 0; m < NM; ++m) Uout[m * plane + cidx] = Uin[m * plane + cidx];
+        return;
+    }
+
+    // 1. stage + cons -> prim.  Tile-corner halo cells are in no stencil: skipped.
+    for (int idx = tid; idx < PW; idx += NT) {
+        const int ly = idx / TXH, lx = idx - ly * TXH;
+        const bool corner = (lx < 2 || lx >= TX + 2) && (ly < 2 || ly >= TY + 2);
+        const int px = gx0 + lx, py = gy0 + ly;        // padded coordinates
+        if (corner || px >= p.nx + 4 || py >= p.ny + 4) continue;
+        double U[NM], W[NM];
+        const double* src = Uin + (size_t)py * p.pitch + px;
+#pragma unroll
+        for (int m = 0; m < NM; ++m) U[m] = src[m * plane];
+        cons2prim14(U, W);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) Ws[m * PW + idx] = W[m];
+    }
+    __syncthreads();
+
+    // 2. x interfaces: interface i of row j lies between tile cells i-1 and i
+    for (int idx = tid; idx < PFX; idx += NT) {
+        const int j = idx / (TX + 1), i = idx - j * (TX + 1);
+        if (gx0 + i > p.nx || gy0 + j >= p.ny) continue;
+        double Fh[NM];
+        interface_flux<NM, false>(p, Ws + (j + 2) * TXH + (i + 2), 1, PW, Fh);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) Fx[m * PFX + idx] = Fh[m];
+    }
+    // 3. y interfaces: interface j of column i lies between tile cells j-1 and j
+    for (int idx = tid; idx < PFY; idx += NT) {
+        const int j = idx / TX, i = idx - j * TX;
+        if (gx0 + i >= p.nx || gy0 + j > p.ny) continue;
+        double Fh[NM];
+        interface_flux<NM, true>(p, Ws + (j + 2) * TXH + (i + 2), TXH, PW, Fh);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) Fy[swap_xy(m) * PFY + idx] = Fh[m];
+    }
+    __syncthreads();
+
+    // 4. update + source + tail reduction
+    double rate = 0.0, speed = 0.0;
+    int bad = 0;
+    if (cell_ok) {
+        const double dtdx = dt / p.dx, dtdy = dt / p.dy;
+        double Un[NM], W[NM];
+#pragma unroll
+        for (int m = 0; m < NM; ++m) {
+            const double* fx = Fx + m * PFX + cj * (TX + 1) + ci;
+            const double* fy = Fy + m * PFY + cj * TX + ci;
+            double v = Uin[m * plane + cidx] - dtdx * (fx[1] - fx[0]);
+            Un[m] = v - dtdy * (fy[TX] - fy[0]);
+            W[m] = Ws[m * PW + (cj + 2) * TXH + ci + 2];
+        }
+        if (p.tau_model != 0)
+            add_source14(W, dt * inv_tau(p, W[0], (W[4] + W[7] + W[9]) / 3.0), Un);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) Uout[m * plane + cidx] = Un[m];
+        cell_rate<NM>(p, Un, rate, speed, bad);
+    }
+    block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
+}
+
+// 5-moment 1-D step: one block = NT consecutive cells, same four stages.
+template <int NT>
+__global__ void __launch_bounds__(NT)
+k_step5(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl, int slot_next)
+{
+    constexpr int NM = 5, PW = NT + 4, PF = NT + 1;
+    __shared__ double Ws[NM * PW];
+    __shared__ double Fx[NM * PF];
+    const int tid = threadIdx.x, gx0 = blockIdx.x * NT;
+    const size_t plane = (size_t)p.rows * p.pitch;
+    const size_t row = (size_t)2 * p.pitch;
+    const double dt = ctrl->dt;
+    const bool cell_ok = gx0 + tid < p.nx;
+    const size_t cidx = row + gx0 + tid + 2;
+    if (ctrl->skip) {
+        if (cell_ok)
+#pragma unroll
+            for (int m = 0; m < NM; ++m) Uout[m * plane + cidx] = Uin[m * plane + cidx];
+        return;
+    }
+    for (int idx = tid; idx < PW; idx += NT) {
+        if (gx0 + idx >= p.nx + 4) continue;
+        double U[NM], W[NM];
+#pragma unroll
+        for (int m = 0; m < NM; ++m) U[m] = Uin[m * plane + row + gx0 + idx];
+        cons2prim5(U, W);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) Ws[m * PW + idx] = W[m];
+    }
+    __syncthreads();
+    for (int idx = tid; idx < PF; idx += NT) {
+        if (gx0 + idx > p.nx) continue;
+        double Fh[NM];
+        interface_flux<NM, false>(p, Ws + idx + 2, 1, PW, Fh);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) Fx[m * PF + idx] = Fh[m];
+    }
+    __syncthreads();
+    double rate = 0.0, speed = 0.0;
+    int bad = 0;
+    if (cell_ok) {
+        const double dtdx = dt / p.dx;
+        double Un[NM], W[NM];
+#pragma unroll
+        for (int m = 0; m < NM; ++m) {
+            Un[m] = Uin[m * plane + cidx] - dtdx * (Fx[m * PF + tid + 1] - Fx[m * PF + tid]);
+            W[m] = Ws[m * PW + tid + 2];
+        }
+        if (p.tau_model != 0) add_source5(W, dt * inv_tau(p, W[0], W[2]), Un);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) Uout[m * plane + cidx] = Un[m];
+        cell_rate<NM>(p, Un, rate, speed, bad);
+    }
+    block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
+}
+
+}  // namespace mm

@@ -1,0 +1,249 @@
+"""Thin ctypes binding of include/mm.h (argument marshalling only).
+
+Every function below forwards to the C-ABI entry point of the same name in libmm.so; device
+memory and the stream come from PyTorch (plumbing).  Nothing here computes any step of the
+method and nothing falls back to a CPU path: a missing library or device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build_ext
+
+SYS5_1D, SYS14_2D = 5, 14
+TAU_NONE, TAU_CONST, TAU_KN = 0, 1, 2
+BC_TRANSMISSIVE, BC_PERIODIC, BC_DIRICHLET = 0, 1, 2
+LIM_NONE, LIM_MINMOD, LIM_VANALBADA = 0, 1, 2
+FLUX_HLL, FLUX_RUSANOV = 0, 1
+OK, EINVAL, EWORKSPACE, ECUDA, ENONFINITE = 0, -1, -2, -3, -4
+MAX_BANDS = 8
+
+EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim", "mm_step",
+           "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
+           "mm_cfl_dt", "mm_launch_count", "mm_destroy", "mm_strerror"]
+
+_dp = C.POINTER(C.c_double)
+
+
+class mm_grid(C.Structure):
+    _fields_ = [("system", C.c_int), ("nx", C.c_int), ("ny", C.c_int),
+                ("x0", C.c_double), ("x1", C.c_double), ("y0", C.c_double), ("y1", C.c_double)]
+
+
+class mm_collision(C.Structure):
+    _fields_ = [("model", C.c_int), ("tau", C.c_double), ("Kn", C.c_double),
+                ("L_ref", C.c_double), ("rho_ref", C.c_double)]
+
+
+class mm_bc(C.Structure):
+    _fields_ = [("type", C.c_int), ("nbands", C.c_int), ("band_lo", _dp), ("band_hi", _dp),
+                ("band_W", _dp), ("default_W", _dp)]
+
+
+class mm_options(C.Structure):
+    _fields_ = [("sigma_lim", C.c_double), ("ws_scale", C.c_double), ("limiter", C.c_int),
+                ("shared_limiter", C.c_int), ("flux", C.c_int), ("stream", C.c_void_p)]
+
+
+class MMError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"mm error {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libmm.so (building it in-tree if the sources are newer).  Raises if impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = build_ext.build()
+    L = C.CDLL(str(path))
+    vp, i, d = C.c_void_p, C.c_int, C.c_double
+    L.mm_workspace_bytes.restype, L.mm_workspace_bytes.argtypes = C.c_size_t, [C.POINTER(mm_grid)]
+    L.mm_create.restype = i
+    L.mm_create.argtypes = [C.POINTER(vp), C.POINTER(mm_grid), C.POINTER(mm_collision),
+                            C.POINTER(mm_bc), C.POINTER(mm_options), vp, C.c_size_t]
+    for name in ("mm_set_state", "mm_set_state_prim", "mm_get_state", "mm_get_state_prim"):
+        f = getattr(L, name)
+        f.restype, f.argtypes = i, [vp, vp, i]
+    L.mm_step.restype, L.mm_step.argtypes = i, [vp, i, d]
+    L.mm_step_fixed_dt.restype, L.mm_step_fixed_dt.argtypes = i, [vp, i, d]
+    L.mm_advance_to.restype, L.mm_advance_to.argtypes = i, [vp, d, d, i]
+    L.mm_get_info.restype = i
+    L.mm_get_info.argtypes = [vp, _dp, C.POINTER(C.c_longlong), _dp, _dp]
+    L.mm_cfl_dt.restype, L.mm_cfl_dt.argtypes = i, [vp, d, _dp]
+    L.mm_launch_count.restype, L.mm_launch_count.argtypes = C.c_longlong, [vp]
+    L.mm_destroy.restype, L.mm_destroy.argtypes = None, [vp]
+    L.mm_strerror.restype, L.mm_strerror.argtypes = C.c_char_p, [i]
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != OK:
+        raise MMError(rc, lib().mm_strerror(rc).decode())
+
+
+def _darr(x, n=None):
+    a = np.ascontiguousarray(x, dtype=np.float64)
+    if n is not None and a.size != n:
+        raise ValueError(f"expected {n} doubles, got {a.size}")
+    return a
+
+
+def mm_workspace_bytes(system: int, nx: int, ny: int = 1, extent=(0.0, 1.0, 0.0, 1.0)) -> int:
+    g = mm_grid(system, nx, ny, *extent)
+    return lib().mm_workspace_bytes(C.byref(g))
+
+
+class Solver:
+    """mm_create ... mm_destroy around a torch-owned workspace.
+
+    `bcs`: 4 dicts (xlo, xhi, ylo, yhi): {"type": BC_*, "bands": [(lo, hi, W), ...], "default": W|None}.
+    State arrays are [nmom][ny][nx]; numpy arrays / CPU tensors go through the host path
+    (on_device = 0), CUDA tensors through the device path (on_device = 1)."""
+
+    def __init__(self, system: int, nx: int, ny: int = 1, extent=(0.0, 1.0, 0.0, 1.0),
+                 collision: Optional[dict] = None, bcs: Optional[Sequence[dict]] = None,
+                 sigma_lim: float = 1e-4, ws_scale: float = 1.0, limiter: int = LIM_MINMOD,
+                 shared_limiter: int = 0, flux: int = FLUX_HLL, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise MMError(ECUDA, "no CUDA device: the moment-method library has no CPU path")
+        L = lib()
+        self._L, self._torch = L, torch
+        self.nm, self.nx, self.ny = system, nx, ny
+        self.device = torch.device(device)
+        g = mm_grid(system, nx, ny, *extent)
+        nbytes = L.mm_workspace_bytes(C.byref(g))
+        if nbytes == 0:
+            raise MMError(EINVAL, "invalid grid")
+        col = collision or {"model": TAU_NONE}
+        c = mm_collision(col.get("model", TAU_NONE), col.get("tau", 0.0), col.get("Kn", 0.0),
+                         col.get("L_ref", 1.0), col.get("rho_ref", 1.0))
+        bcs = list(bcs) if bcs else [{"type": BC_TRANSMISSIVE}] * 4
+        keep, arr = [], (mm_bc * 4)()
+        for k in range(4):
+            b = bcs[k] if k < len(bcs) else {"type": BC_TRANSMISSIVE}
+            bands = b.get("bands", [])
+            lo, hi = _darr([x[0] for x in bands]), _darr([x[1] for x in bands])
+            bw = _darr([x[2] for x in bands]).reshape(-1)
+            dflt = b.get("default")
+            dw = _darr(dflt, system) if dflt is not None else None
+            keep += [lo, hi, bw, dw]
+            arr[k] = mm_bc(b["type"], len(bands), lo.ctypes.data_as(_dp), hi.ctypes.data_as(_dp),
+                           bw.ctypes.data_as(_dp), dw.ctypes.data_as(_dp) if dw is not None else None)
+        with torch.cuda.device(self.device):
+            self._stream = stream if stream is not None else torch.cuda.current_stream()
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) // 256 * 256
+            o = mm_options(sigma_lim, ws_scale, limiter, shared_limiter, flux,
+                           C.c_void_p(self._stream.cuda_stream))
+            h = C.c_void_p()
+            _check(L.mm_create(C.byref(h), C.byref(g), C.byref(c), arr, C.byref(o),
+                               C.c_void_p(self._ws_ptr), nbytes))
+        self._h = h
+        self.workspace_bytes = nbytes
+
+    @classmethod
+    def from_problem(cls, prob: dict, load_state: bool = True, **kw) -> "Solver":
+        s = cls(prob["system"], prob["nx"], prob["ny"], extent=prob["extent"],
+                collision=prob["collision"], bcs=prob["bcs"], **prob["options"], **kw)
+        if load_state:
+            s.set_state_prim(prob["W0"])
+        return s
+
+    # -- state in / out -------------------------------------------------------------
+    def _in(self, x):
+        torch = self._torch
+        n = self.nm * self.ny * self.nx
+        if isinstance(x, torch.Tensor):
+            if x.dtype != torch.float64 or not x.is_contiguous() or x.numel() != n:
+                raise ValueError("state tensor must be contiguous float64 [nmom, ny, nx]")
+            return x, C.c_void_p(x.data_ptr()), int(x.is_cuda)
+        a = _darr(x, n)
+        return a, C.c_void_p(a.ctypes.data), 0
+
+    def set_state(self, U):
+        keep, ptr, dev = self._in(U)
+        _check(self._L.mm_set_state(self._h, ptr, dev))
+        if not dev:
+            self.synchronize()      # the host buffer may go away after this call
+
+    def set_state_prim(self, W):
+        keep, ptr, dev = self._in(W)
+        _check(self._L.mm_set_state_prim(self._h, ptr, dev))
+        if not dev:
+            self.synchronize()
+
+    def _out(self, out, fn):
+        torch = self._torch
+        if out is None:
+            out = np.empty((self.nm, self.ny, self.nx))
+        if isinstance(out, torch.Tensor):
+            keep, ptr, dev = self._in(out)
+        else:
+            if out.dtype != np.float64 or not out.flags.c_contiguous or out.size != self.nm * self.ny * self.nx:
+                raise ValueError("output array must be contiguous float64 [nmom, ny, nx]")
+            ptr, dev = C.c_void_p(out.ctypes.data), 0
+        _check(fn(self._h, ptr, dev))
+        return out
+
+    def get_state(self, out=None):
+        return self._out(out, self._L.mm_get_state)
+
+    def get_state_prim(self, out=None):
+        return self._out(out, self._L.mm_get_state_prim)
+
+    # -- stepping -------------------------------------------------------------------
+    def step(self, n: int, cfl: float):
+        _check(self._L.mm_step(self._h, n, cfl))
+
+    def step_fixed_dt(self, n: int, dt: float):
+        _check(self._L.mm_step_fixed_dt(self._h, n, dt))
+
+    def advance_to(self, t_end: float, cfl: float, max_steps: int = 0):
+        _check(self._L.mm_advance_to(self._h, t_end, cfl, max_steps))
+
+    def cfl_dt(self, cfl: float) -> float:
+        dt = C.c_double()
+        _check(self._L.mm_cfl_dt(self._h, cfl, C.byref(dt)))
+        return dt.value
+
+    def info(self, check: bool = True) -> dict:
+        t, n, dt, sp = C.c_double(), C.c_longlong(), C.c_double(), C.c_double()
+        rc = self._L.mm_get_info(self._h, C.byref(t), C.byref(n), C.byref(dt), C.byref(sp))
+        if check:
+            _check(rc)
+        return {"t": t.value, "steps": n.value, "last_dt": dt.value, "max_speed": sp.value,
+                "status": rc}
+
+    @property
+    def launches(self) -> int:
+        return self._L.mm_launch_count(self._h)
+
+    @property
+    def stream(self):
+        return self._stream
+
+    def synchronize(self):
+        self._stream.synchronize()
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.synchronize()
+            self._L.mm_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,93 @@
+"""CPU-side checks of the product's boundary: the C-ABI library builds for sm_100a, loads without
+a GPU, exports every function include/mm.h declares, validates arguments before touching CUDA,
+and refuses to compute without a device (no CPU fallback).  No compute calls here."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parents[1]
+
+
+@pytest.fixture(scope="module")
+def mm():
+    from paper_2401_15233_b200 import mm as _mm
+    _mm.lib()
+    return _mm
+
+
+def declared_functions():
+    text = (ROOT / "include" / "mm.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mm_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(mm):
+    names = declared_functions()
+    assert len(names) >= 14 and set(names) == set(mm.EXPORTS)
+    lib = mm.lib()
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_binding_structs_match_header(mm):
+    # field order / count of the header structs (layout is plain C, natural alignment)
+    text = (ROOT / "include" / "mm.h").read_text()
+    assert "typedef struct { int system; int nx, ny; double x0, x1, y0, y1; } mm_grid;" in text
+    assert [f[0] for f in mm.mm_grid._fields_] == ["system", "nx", "ny", "x0", "x1", "y0", "y1"]
+    assert [f[0] for f in mm.mm_collision._fields_] == ["model", "tau", "Kn", "L_ref", "rho_ref"]
+    assert [f[0] for f in mm.mm_bc._fields_] == ["type", "nbands", "band_lo", "band_hi", "band_W", "default_W"]
+    assert [f[0] for f in mm.mm_options._fields_] == ["sigma_lim", "ws_scale", "limiter", "shared_limiter", "flux", "stream"]
+    for name, val in [("MM_SYS5_1D", 5), ("MM_SYS14_2D", 14), ("MM_MAX_BANDS", 8)]:
+        assert re.search(rf"{name}\s*=?\s*{val}\b", text)
+
+
+def test_workspace_bytes_and_argument_checks(mm):
+    lib = mm.lib()
+    n = mm.mm_workspace_bytes(14, 2048, 2048)
+    # two padded state copies of 14 planes dominate
+    planes = 2 * 14 * (2048 + 4) * 2064 * 8
+    assert planes <= n <= planes + 16384
+    assert mm.mm_workspace_bytes(5, 1000, 1) > 2 * 5 * 1004 * 5 * 8
+    assert mm.mm_workspace_bytes(5, 10, 2) == 0          # 1-D system needs ny = 1
+    assert mm.mm_workspace_bytes(7, 10, 10) == 0
+    assert mm.mm_workspace_bytes(14, 0, 4) == 0
+    assert lib.mm_strerror(0) == b"ok" and b"invalid" in lib.mm_strerror(-1)
+    # NULL / bad arguments are rejected before any CUDA call
+    g = mm.mm_grid(14, 8, 8, 0, 1, 0, 1)
+    c = mm.mm_collision(0, 0, 0, 1, 1)
+    o = mm.mm_options(1e-4, 1.0, 1, 0, 0, None)
+    b = (mm.mm_bc * 4)()
+    h = C.c_void_p()
+    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(c), b, C.byref(o), None, 0) == mm.EWORKSPACE
+    o.sigma_lim = -1.0
+    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(c), b, C.byref(o), None, 0) == mm.EINVAL
+    assert lib.mm_step(None, 1, 0.4) == mm.EINVAL
+    assert lib.mm_launch_count(None) == 0
+
+
+def test_no_cpu_fallback(mm):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA device present")
+    with pytest.raises(mm.MMError) as e:
+        mm.Solver(14, 8, 8)
+    assert e.value.status == mm.ECUDA
+    # the C entry point itself also refuses: aligned fake workspace, still no device
+    lib = mm.lib()
+    g = mm.mm_grid(5, 8, 1, 0, 1, 0, 1)
+    c = mm.mm_collision(0, 0, 0, 1, 1)
+    o = mm.mm_options(1e-4, 1.0, 1, 0, 0, None)
+    b = (mm.mm_bc * 4)()
+    h = C.c_void_p()
+    n = lib.mm_workspace_bytes(C.byref(g))
+    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(c), b, C.byref(o), C.c_void_p(4096), n) == mm.ECUDA
+    assert b"CUDA" in lib.mm_strerror(mm.ECUDA)
+
+
+def test_product_does_not_touch_the_oracle():
+    for f in (ROOT / "paper_2401_15233_b200").rglob("*"):
+        if f.suffix in (".py", ".cu", ".cuh", ".h"):
+            assert "oracle" not in f.read_text().lower().replace("no cpu", ""), f
+    assert "mmo" not in (ROOT / "include" / "mm.h").read_text()

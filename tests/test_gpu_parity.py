@@ -1,0 +1,248 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element, on the same seeded inputs (mm_workloads.py).
+
+Bar (BASELINE.json north_star): per moment k,
+    max_cells |U_gpu - U_oracle| / max_cells |U_oracle| <= 1e-10  after 100 steps at fixed dt,
+and a moment that is identically zero in the oracle is identically zero on the GPU.
+"""
+import numpy as np
+import pytest
+
+import mm_workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def mm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2401_15233_b200 import mm as _mm
+    _mm.lib()
+    return _mm
+
+
+def oracle_solver(mmo, prob, **kw):
+    s = mmo.Solver(prob["system"], prob["nx"], prob["ny"], extent=prob["extent"],
+                   collision=prob["collision"], bcs=prob["bcs"], nthreads=0, **prob["options"], **kw)
+    s.set_state_prim(prob["W0"])
+    return s
+
+
+def rel_err(Ug, Uo):
+    """per-moment max-norm relative error; checks exact zeros."""
+    errs = []
+    for m in range(Uo.shape[0]):
+        scale = np.abs(Uo[m]).max()
+        if scale == 0.0:
+            assert np.all(Ug[m] == 0.0), f"moment {m}: oracle identically 0, GPU not"
+            errs.append(0.0)
+        else:
+            errs.append(np.abs(Ug[m] - Uo[m]).max() / scale)
+    return np.array(errs)
+
+
+def assert_parity(Ug, Uo, tol=TOL):
+    assert np.all(np.isfinite(Uo)), "oracle state is not finite: test case is ill-posed"
+    assert np.all(np.isfinite(Ug))
+    e = rel_err(Ug, Uo)
+    assert e.max() <= tol, f"per-moment rel. error {e}"
+    return e
+
+
+def run_both(mm, mmo, prob, nsteps, dt=None, cfl=0.4, dt_frac=0.5):
+    so = oracle_solver(mmo, prob)
+    sg = mm.Solver.from_problem(prob)
+    if dt is None:
+        dt = dt_frac * so.cfl_dt(cfl)
+    so.step_fixed_dt(nsteps, dt)
+    sg.step_fixed_dt(nsteps, dt)
+    Ug, Uo = sg.get_state(), so.get_state()
+    info = sg.info()
+    assert info["steps"] == nsteps
+    assert info["t"] == pytest.approx(so.info()["t"], rel=1e-13)
+    return Ug, Uo
+
+
+# ----------------------------------------------------------- state in / out, set-up values
+def test_state_roundtrip_and_prim_conversion(mm, mmo):
+    prob = wl.random_smooth14(70, 37)
+    sg = mm.Solver.from_problem(prob)
+    so = oracle_solver(mmo, prob)
+    Uo = so.get_state()
+    assert_parity(sg.get_state(), Uo, 1e-14)                    # prim -> cons on the GPU
+    assert_parity(sg.get_state_prim(), prob["W0"], 1e-13)      # and back
+    sg.set_state(Uo)
+    assert np.array_equal(sg.get_state(), Uo)                   # conserved in/out is a copy
+    import torch
+    Ud = torch.from_numpy(Uo).cuda()
+    sg.set_state(Ud)
+    out = torch.empty_like(Ud)
+    sg.get_state(out)
+    assert torch.equal(out, Ud)
+    assert sg.cfl_dt(0.4) == pytest.approx(so.cfl_dt(0.4), rel=1e-13)
+    assert sg.info()["max_speed"] > 0
+
+    p5 = wl.random_smooth5(333)
+    s5 = mm.Solver.from_problem(p5); o5 = oracle_solver(mmo, p5)
+    assert_parity(s5.get_state(), o5.get_state(), 1e-14)
+    assert s5.cfl_dt(0.5) == pytest.approx(o5.cfl_dt(0.5), rel=1e-13)
+
+
+def test_cfl_dt_includes_dirichlet_ghosts(mm, mmo):
+    prob = wl.crossed_jets(64, Kn=1.0)
+    sg = mm.Solver.from_problem(prob); so = oracle_solver(mmo, prob)
+    # the jets' ghost states are the fastest cells of the initial state (R13)
+    assert sg.cfl_dt(0.4) == pytest.approx(so.cfl_dt(0.4), rel=1e-13)
+    bg = dict(prob, bcs=[dict(type=wl.BC_TRANSMISSIVE)] * 4)
+    assert mm.Solver.from_problem(bg).cfl_dt(0.4) > 2.0 * sg.cfl_dt(0.4)
+
+
+# ----------------------------------------------------------------- small, all the variants
+@pytest.mark.parametrize("limiter,shared,flux", [
+    (wl.LIM_MINMOD, 0, wl.FLUX_HLL), (wl.LIM_MINMOD, 1, wl.FLUX_RUSANOV),
+    (wl.LIM_VANALBADA, 0, wl.FLUX_RUSANOV), (wl.LIM_VANALBADA, 1, wl.FLUX_HLL),
+    (wl.LIM_NONE, 0, wl.FLUX_HLL)])
+@pytest.mark.parametrize("Kn", [None, 0.05])
+def test_smooth14_periodic_variants(mm, mmo, limiter, shared, flux, Kn):
+    # 70 x 37: several 32 x 8 tiles and a ragged tail in both directions; all 14 primitives vary
+    prob = wl.random_smooth14(70, 37, Kn=Kn, limiter=limiter, shared_limiter=shared, flux=flux)
+    Ug, Uo = run_both(mm, mmo, prob, 30)
+    assert_parity(Ug, Uo)
+
+
+def test_smooth14_transmissive(mm, mmo):
+    prob = wl.random_smooth14(45, 19, Kn=0.2, periodic=False)
+    Ug, Uo = run_both(mm, mmo, prob, 40)
+    assert_parity(Ug, Uo)
+
+
+@pytest.mark.parametrize("nx,ny", [(1, 1), (3, 2), (5, 1), (33, 9)])
+def test_tiny_grids(mm, mmo, nx, ny):
+    prob = wl.random_smooth14(nx, ny, Kn=0.3)
+    Ug, Uo = run_both(mm, mmo, prob, 10)
+    assert_parity(Ug, Uo)
+
+
+@pytest.mark.parametrize("limiter,flux", [(wl.LIM_MINMOD, wl.FLUX_HLL), (wl.LIM_VANALBADA, wl.FLUX_RUSANOV)])
+def test_smooth5_periodic(mm, mmo, limiter, flux):
+    prob = wl.random_smooth5(333, Kn=0.05, limiter=limiter, flux=flux)
+    Ug, Uo = run_both(mm, mmo, prob, 100, cfl=0.5)
+    assert_parity(Ug, Uo)
+
+
+# ------------------------------------------------------------------- BASELINE configs
+def test_C1_sod5_100_steps_fixed_dt(mm, mmo):
+    prob = wl.sod5(1000, Kn=0.01)
+    Ug, Uo = run_both(mm, mmo, prob, 100, cfl=0.5)
+    assert_parity(Ug, Uo)
+
+
+def test_C1_sod5_to_t02_with_cfl_steps(mm, mmo):
+    """Whole run with each side's own CFL dt (dt differs in the last bits, so the bar is looser)."""
+    prob = wl.sod5(1000, Kn=0.01)
+    so = oracle_solver(mmo, prob); sg = mm.Solver.from_problem(prob)
+    so.advance_to(0.2, 0.5); sg.advance_to(0.2, 0.5)
+    ig, io = sg.info(), so.info()
+    assert ig["t"] == 0.2 and ig["steps"] == io["steps"]
+    assert_parity(sg.get_state(), so.get_state(), 1e-8)
+
+
+@pytest.mark.parametrize("Kn", [1e-3, 1e-2, 1e-1, 1.0])
+def test_C2_sod14_4096x4(mm, mmo, Kn):
+    prob = wl.sod14(4096, 4, Kn=Kn)
+    Ug, Uo = run_both(mm, mmo, prob, 100, cfl=0.5)
+    assert_parity(Ug, Uo)
+    for j in range(1, 4):
+        assert np.array_equal(Ug[:, j], Ug[:, 0])
+
+
+def test_C3_jets_512_from_t0(mm, mmo):
+    prob = wl.crossed_jets(512, Kn=1.0)
+    Ug, Uo = run_both(mm, mmo, prob, 100, cfl=0.4)
+    assert_parity(Ug, Uo)
+
+
+def test_C3_jets_developed_state(mm, mmo):
+    """Developed state (jets have crossed): produced by the ORACLE with CFL stepping on a
+    128^2 grid, then used as the common input of 100 fixed-dt steps."""
+    prob = wl.crossed_jets(128, Kn=1.0)
+    so = oracle_solver(mmo, prob)
+    so.advance_to(0.15, 0.4)
+    U0 = so.get_state()
+    dt = 0.5 * so.cfl_dt(0.4)
+    sg = mm.Solver.from_problem(prob, load_state=False)
+    sg.set_state(U0)
+    so.set_state(U0)
+    so.step_fixed_dt(100, dt); sg.step_fixed_dt(100, dt)
+    assert_parity(sg.get_state(), so.get_state())
+    # CFL stepping from the same state: same number of steps to the same time
+    so.set_state(U0); sg.set_state(U0)
+    so.step(20, 0.4); sg.step(20, 0.4)
+    assert sg.info()["t"] == pytest.approx(so.info()["t"], rel=1e-12)
+    assert_parity(sg.get_state(), so.get_state(), 1e-9)
+
+
+def test_C4_jets_2048_sampled_windows(mm, mmo):
+    """Full bench size, bench launch configuration: after n steps a cell depends only on the
+    (2n)-neighbourhood of its initial data, so the oracle is run on small windows of the same
+    seeded state (transmissive window edges) and compared on the cells no edge can have reached."""
+    n, nsteps, half, margin = 2048, 3, 14, 2 * 3 + 1
+    prob = wl.crossed_jets(n, Kn=0.1, perturb=0.01)
+    sg = mm.Solver.from_problem(prob)
+    so_dt = 0.5 * sg.cfl_dt(0.4)
+    sg.step_fixed_dt(nsteps, so_dt)
+    Ug = sg.get_state()
+    W0 = prob["W0"]
+    rng = np.random.default_rng(7)
+    centres = [(int(a), int(b)) for a, b in rng.integers(half, n - half, size=(6, 2))]
+    centres += [(half, int(0.35 * n)), (half, int(0.65 * n)), (half, int(0.5 * n))]   # at the inflow side
+    h = 1.0 / n
+    for (ci, cj) in centres:
+        i0, j0 = ci - half, cj - half
+        w = 2 * half
+        sub = dict(prob, nx=w, ny=w, W0=np.ascontiguousarray(W0[:, j0:j0 + w, i0:i0 + w]),
+                   extent=(i0 * h, (i0 + w) * h, j0 * h, (j0 + w) * h))
+        if i0 > 0:
+            sub["bcs"] = [dict(type=wl.BC_TRANSMISSIVE)] * 4
+        so = oracle_solver(mmo, sub)
+        so.step_fixed_dt(nsteps, so_dt)
+        Uo = so.get_state()
+        lo_i = 0 if i0 == 0 else margin
+        sl = (slice(None), slice(margin, w - margin), slice(lo_i, w - margin))
+        ref = Uo[sl]
+        got = Ug[:, j0:j0 + w, i0:i0 + w][sl]
+        scale = np.abs(Ug).max(axis=(1, 2))
+        for m in range(14):
+            if np.all(ref[m] == 0):
+                assert np.all(got[m] == 0)
+            else:
+                assert np.abs(got[m] - ref[m]).max() <= TOL * scale[m], (ci, cj, m)
+
+
+# ------------------------------------------------------------------------ error behaviour
+def test_errors_and_failure_flag(mm, mmo):
+    with pytest.raises(mm.MMError) as e:
+        mm.Solver(14, 8, 8, sigma_lim=0.0)
+    assert e.value.status == mm.EINVAL
+    with pytest.raises(mm.MMError):
+        mm.Solver(5, 8, 2)
+    with pytest.raises(mm.MMError):
+        mm.Solver(14, 8, 8, bcs=[dict(type=wl.BC_PERIODIC), dict(type=wl.BC_TRANSMISSIVE)] * 2)
+    prob = wl.random_smooth14(16, 16)
+    s = mm.Solver.from_problem(prob, load_state=False)
+    with pytest.raises(mm.MMError):
+        s.step(1, 0.4)                                 # no state yet
+    s.set_state_prim(prob["W0"])
+    s.step(0, 0.4)                                     # empty request is a no-op
+    assert s.info()["steps"] == 0
+    W = prob["W0"].copy()
+    W[4, 3, 3] = W[7, 3, 3] = W[9, 3, 3] = -1.0        # negative pressure
+    s.set_state_prim(W)
+    U0 = s.get_state()
+    s.step(3, 0.4)
+    inf = s.info(check=False)
+    assert inf["status"] == mm.ENONFINITE and inf["steps"] == 0
+    assert np.array_equal(s.get_state(), U0)           # state left as is for inspection
