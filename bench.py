@@ -1,0 +1,272 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s of the 14-moment 2-D time step on the crossed-jet workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 2048] [--kn 0.1]
+
+A "step" is one pass of the whole hot path (ghost cells, cons->prim, MUSCL, closure fluxes +
+wave speeds, HLL, update + BGK source, CFL reduction -> next dt) over BASELINE.json configs[3]:
+2048 x 2048 cells, crossed Mach-3 jets, Kn = 0.1, seeded +-1% density perturbation, CFL 0.4.
+Prints ONE JSON line (rank 0).  See DESIGN.md section 9 for how each field is obtained.
+
+N > 1 (torchrun): the path has no multi-GPU exchange yet ("replicas only"):
+every rank steps its own replica, value = all ranks' cell updates / max-over-ranks time.
+`--impl reference` times the CPU oracle (test infrastructure) on a bounded sample instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import mm_workloads as wl  # noqa: E402
+
+METRIC = "cell-updates/s (fp64, 14-moment 2-D)"
+UNIT = "cell-updates/s"
+CFL = 0.4
+
+
+def flops_per_cell_update(shared_limiter: bool):
+    """Algorithmic FP64 operations per cell update (each + - * / sqrt exp log = 1).
+    -> (count of the formulation the CUDA path runs, count of the oracle's naive restatement).
+    The roofline line uses the FIRST (smaller) number: flops the kernel does not execute are not
+    credited to it.  Both are produced by committed counting builds, not typed in."""
+    from paper_2401_15233_b200 import build_ext
+    k = build_ext.read_opcount()["kernel_flops_per_cell_update_14_"
+                                 + ("shared_limiter" if shared_limiter else "per_variable_limiter")]
+    o = None
+    for line in (ROOT / "tests" / "golden" / "oracle_opcount.txt").read_text().splitlines():
+        if line.startswith("flops_per_cell_update_14 "):
+            o = float(line.split()[1])
+    return float(k), o
+
+
+def peaks() -> dict:
+    f = ROOT / "MEASURED_PEAKS.json"
+    return json.loads(f.read_text()) if f.exists() else {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.th.join(timeout=2)
+
+    def summary(self) -> dict:
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        busy = [c for c in sm if c > 0.5 * max(sm)] if sm else []
+        return {"sm_mhz": float(np.median(busy)) if busy else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def workload(n: int, kn: float) -> dict:
+    return wl.crossed_jets(n, Kn=kn, perturb=0.01)
+
+
+def time_oracle(n: int, kn: float, steps: int, warmup: int = 0, nthreads: int = 0):
+    """Oracle (as it stands) on an n x n instance of the workload: cell-updates/s, threads."""
+    from oracle import mmo
+    prob = workload(n, kn)
+    so = mmo.Solver(prob["system"], prob["nx"], prob["ny"], extent=prob["extent"],
+                    collision=prob["collision"], bcs=prob["bcs"], nthreads=nthreads, **prob["options"])
+    so.set_state_prim(prob["W0"])
+    if warmup:
+        so.step(warmup, CFL)
+    t0 = time.perf_counter()
+    so.step(steps, CFL)
+    dt = time.perf_counter() - t0
+    return n * n * steps / dt, so.threads, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = args.ref_n
+    val, threads, secs = time_oracle(n, args.kn, args.steps, args.warmup)
+    sample = f"{n}x{n} instance of the crossed-jet workload, {args.steps} CFL steps ({secs:.1f} s)"
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1),
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "gpu_launches": 0,
+           "config": {"workload": f"crossed jets 2048x2048 Kn={args.kn} (BASELINE configs[3]); "
+                                  f"oracle timed on a bounded {n}x{n} sample of it"},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out), flush=True)
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2401_15233_b200 import mm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the library has no CPU path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    n, K, W = args.n, args.steps, args.warmup
+    prob = workload(n, args.kn)
+    cells = n * n
+    s = mm.Solver.from_problem(prob, load_state=False, device=f"cuda:{local}")
+    nbytes_state = 14 * cells * 8
+    W_host = torch.from_numpy(prob["W0"]).pin_memory()
+    U_host = torch.empty((14, n, n), dtype=torch.float64).pin_memory()
+    W_dev = W_host.to(f"cuda:{local}")
+
+    # ---- device-resident timing: K steps, inputs in HBM (two 470 MB copies >> 126 MB L2)
+    s.set_state_prim(W_dev)
+    s.step(W, CFL)
+    barrier()
+    l0 = s.launches
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        s.profile_begin()
+        ev0.record(s.stream)
+        s.step(K, CFL)
+        ev1.record(s.stream)
+        barrier()
+        kern_ms, kern_n = s.profile_end()
+    ms = ev0.elapsed_time(ev1)
+    launches = s.launches - l0
+    info = s.info()
+    if world > 1:
+        t = torch.tensor([ms], device=f"cuda:{local}", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * cells * K / (ms * 1e-3)
+
+    # ---- end to end through the API with HOST buffers: H2D of the state, K steps, D2H of the result
+    barrier()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(s.stream)
+    s.set_state_prim(W_host)
+    s.step(K, CFL)
+    s.get_state(U_host)
+    e1.record(s.stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=f"cuda:{local}", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = world * cells * K / (e2e_ms * 1e-3)
+    finite = bool(torch.isfinite(U_host).all())
+
+    if rank == 0:
+        fpc, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]))
+        peak_tf = mm.mm_measure_fp64_peak(5)
+        kern_avg_ms = kern_ms / max(kern_n, 1)
+        achieved_tf = fpc * cells / (kern_avg_ms * 1e-3) * 1e-12
+        pk = peaks()
+        hbm_gbs = 224.0 * cells / (kern_avg_ms * 1e-3) * 1e-9
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            v, threads, secs = time_oracle(args.ref_n, args.kn, args.cpu_steps)
+            cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                   "sample": f"{args.ref_n}x{args.ref_n} instance of the same workload, "
+                             f"{args.cpu_steps} CFL steps ({secs:.1f} s)"}
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"crossed jets {n}x{n}, 14-moment, Kn={args.kn}, +-1% seeded density "
+                                   f"perturbation, minmod (shared psi) + HLL, CFL {CFL} (BASELINE configs[3])",
+                       "cells": cells, "l2": "inputs larger than L2 (2 x 470 MB state copies)",
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "t_end": info["t"], "state_finite": finite},
+            "clocks": clk.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes_state / K,
+                    "d2h_bytes_per_step": nbytes_state / K,
+                    "note": f"one job = H2D of the {nbytes_state} B state from pinned memory + {K} steps + "
+                            f"D2H of the result; bytes amortised over the {K} steps"},
+            "gpu_launches": launches,
+            "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                         "frac": achieved_tf / peak_tf if peak_tf else None, "traffic": None,
+                         "kernel": "k_step14", "kernel_ms": kern_avg_ms,
+                         "flops_per_cell_update": fpc, "flops_per_cell_update_oracle": fpc_oracle,
+                         "peak_source": "FP64 DFMA loop measured in this run (mm_measure_fp64_peak)",
+                         "hbm_algorithmic_gbs": hbm_gbs, "hbm_peak_gbs": pk.get("hbm_gbs"),
+                         "hbm_frac": hbm_gbs / pk["hbm_gbs"] if pk.get("hbm_gbs") else None},
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--n", type=int, default=2048)
+    ap.add_argument("--kn", type=float, default=0.1)
+    ap.add_argument("--ref-n", type=int, default=256, help="grid of the bounded oracle sample")
+    ap.add_argument("--cpu-steps", type=int, default=40)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -117,6 +117,17 @@ int mm_cfl_dt(mm_solver *s, double cfl, double *dt);
 /* Number of kernel launches enqueued by this solver so far. */
 long long mm_launch_count(const mm_solver *s);
 
+/* Measurement hooks (used by bench.py for the roofline line).
+ * Between mm_profile_begin and mm_profile_end every launch of the fused step kernel is
+ * bracketed by CUDA events on the solver's stream; mm_profile_end synchronises and returns the
+ * summed device time of those launches (milliseconds) and their number. */
+int mm_profile_begin(mm_solver *s);
+int mm_profile_end(mm_solver *s, double *step_kernel_ms, long long *launches);
+/* FP64 FMA peak of the current device, measured with a register-resident DFMA loop on
+ * `stream` (cudaStream_t): 2 flop per FMA, best of `repeats` launches.  This is the roofline
+ * denominator of this FP64-ALU-bound method; MEASURED_PEAKS.json has no FP64 entry. */
+int mm_measure_fp64_peak(void *stream, int repeats, double *tflops);
+
 void mm_destroy(mm_solver *s);
 const char *mm_strerror(int status);
 

@@ -95,7 +95,10 @@ def crossed_jets(n: int = 512, Kn: float = 1.0, perturb: float = 0.0, mach: floa
     y in [0.3,0.4] (+angle) and [0.6,0.7] (-angle) into a background rho_bg, T = 1; the rest of
     the left side is held at the background, the other sides are transmissive.  Speed uses
     a = sqrt(gamma R T) with gamma = 5/3.  `perturb` = relative amplitude of
-    the uniform random density perturbation of the initial background (T = 1 kept, so P = rho)."""
+    the uniform random density perturbation of the initial background (T = 1 kept, so P = rho).
+    The limiter value is shared by all primitives unless overridden: with
+    per-variable limiting this problem loses positivity within a few steps (R14)."""
+    options.setdefault("shared_limiter", 1)
     speed = mach * math.sqrt(5.0 / 3.0)
     th = math.radians(angle_deg)
     jet_lo = maxwellian(SYS14, 1.0, (speed * math.cos(th), speed * math.sin(th), 0.0), 1.0)

@@ -69,7 +69,12 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    L = C.CDLL(str(build()))
+    _lib = bind(C.CDLL(str(build())))
+    return _lib
+
+
+def bind(L):
+    """Attach the argument / result types of oracle/mmo.h to a loaded library."""
     d, i, p = C.c_double, C.c_int, _dp
     sig = {
         "mmo_cons2prim5": (None, [p, p]), "mmo_prim2cons5": (None, [p, p]),
@@ -102,7 +107,6 @@ def lib():
     for name, (res, args) in sig.items():
         f = getattr(L, name)
         f.restype, f.argtypes = res, args
-    _lib = L
     return L
 
 

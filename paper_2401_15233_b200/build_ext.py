@@ -42,3 +42,29 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
 if __name__ == "__main__":
     print(build(force=True, verbose=True))
+
+
+OPCOUNT_TXT = PKG / "opcount.txt"
+
+
+def opcount(write: bool = True) -> dict:
+    """Source-level FP64 operations per cell update of the CUDA path (csrc/opcount_host.cpp:
+    mm_physics.cuh compiled on the host with a counting type).  Writes opcount.txt."""
+    import tempfile
+    with tempfile.TemporaryDirectory() as td:
+        exe = Path(td) / "opcount_host"
+        subprocess.run(["g++", "-std=c++17", "-O1", "-w", "-o", str(exe), str(CSRC / "opcount_host.cpp")],
+                       check=True, cwd=CSRC)
+        out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
+    vals = {ln.split()[0]: int(ln.split()[1]) for ln in out.splitlines() if ln.strip()}
+    if write:
+        head = ("# FP64 operations per cell update of the CUDA path, counted at source level by\n"
+                "# `python -c 'from paper_2401_15233_b200 import build_ext; build_ext.opcount()'`\n"
+                "# (csrc/opcount_host.cpp; each + - * / sqrt exp log = 1, FMA = 2; no tile overhead).\n")
+        OPCOUNT_TXT.write_text(head + out)
+    return vals
+
+
+def read_opcount() -> dict:
+    return {ln.split()[0]: int(ln.split()[1]) for ln in OPCOUNT_TXT.read_text().splitlines()
+            if ln.strip() and not ln.startswith("#")}

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 using namespace mm;
 
@@ -60,6 +61,8 @@ struct mm_solver {
     int has_state;
     long long launches;
     size_t smem14;
+    bool profiling;
+    std::vector<cudaEvent_t> ev;   // start/stop pairs around the step kernel while profiling
 };
 
 namespace {
@@ -88,18 +91,27 @@ int launch_ghost(mm_solver* s, const StepCtl& sc, int finalize)
 int launch_step(mm_solver* s, const StepCtl& sc)
 {
     int rc;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (s->profiling) {
+        MM_CUDA(cudaEventCreate(&e0));
+        MM_CUDA(cudaEventCreate(&e1));
+        s->ev.push_back(e0); s->ev.push_back(e1);
+    }
     if (s->L.nm == 5) {
         if ((rc = launch_ghost<5>(s, sc, 1))) return rc;
         const int nb = (s->p.nx + kNT5 - 1) / kNT5;
+        if (e0) MM_CUDA(cudaEventRecord(e0, s->stream));
         k_step5<kNT5><<<nb, kNT5, 0, s->stream>>>(s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1);
         MM_LAUNCHED(s, "k_step5");
     } else {
         if ((rc = launch_ghost<14>(s, sc, 1))) return rc;
         dim3 grid((s->p.nx + kTX - 1) / kTX, (s->p.ny + kTY - 1) / kTY);
+        if (e0) MM_CUDA(cudaEventRecord(e0, s->stream));
         k_step14<kTX, kTY><<<grid, kTX * kTY, s->smem14, s->stream>>>(
             s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1);
         MM_LAUNCHED(s, "k_step14");
     }
+    if (e1) MM_CUDA(cudaEventRecord(e1, s->stream));
     s->cur ^= 1;
     s->slot ^= 1;
     return MM_OK;
@@ -357,7 +369,69 @@ int mm_cfl_dt(mm_solver* s, double cfl, double* dt)
 
 long long mm_launch_count(const mm_solver* s) { return s ? s->launches : 0; }
 
-void mm_destroy(mm_solver* s) { delete s; }
+int mm_profile_begin(mm_solver* s)
+{
+    if (!s) return MM_EINVAL;
+    for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
+    s->ev.clear();
+    s->profiling = true;
+    return MM_OK;
+}
+
+int mm_profile_end(mm_solver* s, double* step_kernel_ms, long long* launches)
+{
+    if (!s || !s->profiling) return MM_EINVAL;
+    s->profiling = false;
+    MM_CUDA(cudaStreamSynchronize(s->stream));
+    double total = 0.0;
+    for (size_t k = 0; k + 1 < s->ev.size(); k += 2) {
+        float ms = 0.f;
+        MM_CUDA(cudaEventElapsedTime(&ms, s->ev[k], s->ev[k + 1]));
+        total += ms;
+    }
+    if (step_kernel_ms) *step_kernel_ms = total;
+    if (launches) *launches = (long long)(s->ev.size() / 2);
+    for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
+    s->ev.clear();
+    return MM_OK;
+}
+
+int mm_measure_fp64_peak(void* stream, int repeats, double* tflops)
+{
+    if (!tflops || repeats < 1) return MM_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    MM_CUDA(cudaGetDevice(&dev));
+    MM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* d_out = nullptr;
+    MM_CUDA(cudaMalloc(&d_out, sizeof(double)));      // measurement scratch only, not solver memory
+    cudaEvent_t e0, e1;
+    MM_CUDA(cudaEventCreate(&e0));
+    MM_CUDA(cudaEventCreate(&e1));
+    const int iters = 20000, blocks = sms * 8, threads = 256;
+    double best = 0.0;
+    for (int r = 0; r < repeats + 1; ++r) {            // first launch is the warm-up
+        cudaEventRecord(e0, st);
+        k_dfma_peak<<<blocks, threads, 0, st>>>(d_out, iters, 0.999999, 1e-6);
+        cudaEventRecord(e1, st);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(d_out); return cuda_fail(e, "k_dfma_peak"); }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double tf = 2.0 * 16.0 * (double)iters * blocks * threads / (ms * 1e-3) * 1e-12;
+        if (r > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    *tflops = best;
+    return MM_OK;
+}
+
+void mm_destroy(mm_solver* s)
+{
+    if (!s) return;
+    for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
+    delete s;
+}
 
 const char* mm_strerror(int status)
 {

@@ -448,4 +448,20 @@ k_step5(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctr
     block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
 }
 
+// Register-resident DFMA loop: 16 independent chains per thread, 2 flop per FMA.
+__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a, double b)
+{
+    double x[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) x[k] = (double)(threadIdx.x + k) * 1e-3;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) x[k] = fma(x[k], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s += x[k];
+    if (s == 123.456) out[0] = s;       // never true: keeps the loop alive
+}
+
 }  // namespace mm

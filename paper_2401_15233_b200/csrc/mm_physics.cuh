@@ -5,8 +5,10 @@
 // powers of the pressure tensor use the Cayley-Hamilton identity instead of matrix products.
 // The y direction reuses the x routines on index-swapped states (L414).
 #pragma once
+#ifndef MM_OPCOUNT_HOST          // csrc/opcount_host.cpp compiles this header on the host instead
 #include <cuda_runtime.h>
 #include <math.h>
+#endif
 
 namespace mm {
 

@@ -23,7 +23,8 @@ MAX_BANDS = 8
 
 EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim", "mm_step",
            "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
-           "mm_cfl_dt", "mm_launch_count", "mm_destroy", "mm_strerror"]
+           "mm_cfl_dt", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
+           "mm_measure_fp64_peak", "mm_destroy", "mm_strerror"]
 
 _dp = C.POINTER(C.c_double)
 
@@ -79,6 +80,10 @@ def lib() -> C.CDLL:
     L.mm_get_info.argtypes = [vp, _dp, C.POINTER(C.c_longlong), _dp, _dp]
     L.mm_cfl_dt.restype, L.mm_cfl_dt.argtypes = i, [vp, d, _dp]
     L.mm_launch_count.restype, L.mm_launch_count.argtypes = C.c_longlong, [vp]
+    L.mm_profile_begin.restype, L.mm_profile_begin.argtypes = i, [vp]
+    L.mm_profile_end.restype = i
+    L.mm_profile_end.argtypes = [vp, _dp, C.POINTER(C.c_longlong)]
+    L.mm_measure_fp64_peak.restype, L.mm_measure_fp64_peak.argtypes = i, [vp, i, _dp]
     L.mm_destroy.restype, L.mm_destroy.argtypes = None, [vp]
     L.mm_strerror.restype, L.mm_strerror.argtypes = C.c_char_p, [i]
     _lib = L
@@ -100,6 +105,15 @@ def _darr(x, n=None):
 def mm_workspace_bytes(system: int, nx: int, ny: int = 1, extent=(0.0, 1.0, 0.0, 1.0)) -> int:
     g = mm_grid(system, nx, ny, *extent)
     return lib().mm_workspace_bytes(C.byref(g))
+
+
+def mm_measure_fp64_peak(repeats: int = 5, stream=None) -> float:
+    """Measured FP64 FMA peak of the current device in TFLOP/s (2 flop per FMA)."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    tf = C.c_double()
+    _check(lib().mm_measure_fp64_peak(C.c_void_p(st.cuda_stream), repeats, C.byref(tf)))
+    return tf.value
 
 
 class Solver:
@@ -224,6 +238,15 @@ class Solver:
             _check(rc)
         return {"t": t.value, "steps": n.value, "last_dt": dt.value, "max_speed": sp.value,
                 "status": rc}
+
+    def profile_begin(self):
+        _check(self._L.mm_profile_begin(self._h))
+
+    def profile_end(self):
+        """-> (summed device time of the fused step kernel in ms, number of its launches)."""
+        ms, n = C.c_double(), C.c_longlong()
+        _check(self._L.mm_profile_end(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
 
     @property
     def launches(self) -> int:
