@@ -2,6 +2,7 @@
 // kernel launches.  No arithmetic of the method runs here; there is no CPU fallback.
 #include "../../include/mm.h"
 #include "mm_kernels.cuh"
+#include "mm_strip14.cuh"
 
 #include <cstdio>
 #include <cstring>
@@ -12,7 +13,6 @@ using namespace mm;
 
 namespace {
 
-constexpr int kTX = 32, kTY = 8;        // 14-moment tile (cells per block)
 constexpr int kNT5 = 128;               // 5-moment cells per block
 constexpr int kRateNT = 256;
 
@@ -45,6 +45,23 @@ bool make_layout(const mm_grid* g, Layout* L)
     return true;
 }
 
+// Strips are 31 cells wide; rows are cut into nchunks chunks so that the nstrips * nchunks warp
+// items fill whole waves of the `slots` resident warps.  A chunk of n rows costs n + ~0.8 row
+// passes (one extra y-interface row and three extra row conversions).
+void choose_decomposition(int nx, int ny, int slots, int* nstrips, int* nchunks)
+{
+    const int ns = (nx + kSW - 1) / kSW;
+    double best = 1e300;
+    int bestc = 1;
+    for (int c = 1; c <= ny; ++c) {
+        const int rows = (ny + c - 1) / c;
+        const long long waves = ((long long)ns * c + slots - 1) / slots;
+        const double cost = (double)waves * (rows + 0.8);
+        if (cost < best * (1.0 - 1e-9)) { best = cost; bestc = c; }
+    }
+    *nstrips = ns; *nchunks = bestc;
+}
+
 }  // namespace
 
 struct mm_solver {
@@ -61,6 +78,7 @@ struct mm_solver {
     int has_state;
     long long launches;
     size_t smem14;
+    int nstrips, nchunks;   // 14-moment work decomposition (mm_strip14.cuh)
     bool profiling;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the step kernel while profiling
 };
@@ -105,11 +123,11 @@ int launch_step(mm_solver* s, const StepCtl& sc)
         MM_LAUNCHED(s, "k_step5");
     } else {
         if ((rc = launch_ghost<14>(s, sc, 1))) return rc;
-        dim3 grid((s->p.nx + kTX - 1) / kTX, (s->p.ny + kTY - 1) / kTY);
+        const int items = s->nstrips * s->nchunks;
         if (e0) MM_CUDA(cudaEventRecord(e0, s->stream));
-        k_step14<kTX, kTY><<<grid, kTX * kTY, s->smem14, s->stream>>>(
-            s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1);
-        MM_LAUNCHED(s, "k_step14");
+        k_step14_strip<<<(items + kStripWPB - 1) / kStripWPB, 32 * kStripWPB, s->smem14, s->stream>>>(
+            s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks);
+        MM_LAUNCHED(s, "k_step14_strip");
     }
     if (e1) MM_CUDA(cudaEventRecord(e1, s->stream));
     s->cur ^= 1;
@@ -258,10 +276,14 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
     delete hb;
     if (e != cudaSuccess) { delete s; return cuda_fail(e, "mm_create workspace init"); }
 
-    s->smem14 = (size_t)14 * ((kTY + 4) * (kTX + 4) + kTY * (kTX + 1) + (kTY + 1) * kTX) * sizeof(double);
+    s->smem14 = (size_t)kStripWPB * kWarpSmemD * sizeof(double);
     if (nm == 14) {
-        e = cudaFuncSetAttribute(k_step14<kTX, kTY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->smem14);
-        if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaFuncSetAttribute(k_step14)"); }
+        e = cudaFuncSetAttribute(k_step14_strip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->smem14);
+        if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaFuncSetAttribute(k_step14_strip)"); }
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        choose_decomposition(grid->nx, grid->ny, sms * 8, &s->nstrips, &s->nchunks);
         k_bc_table<14><<<4, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 4);
     } else {
         k_bc_table<5><<<2, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 2);

@@ -193,24 +193,41 @@ def test_C3_jets_512_from_t0(mm, mmo):
 
 def test_C3_jets_developed_state(mm, mmo):
     """Developed state (jets have crossed): produced by the ORACLE with CFL stepping on a
-    128^2 grid, then used as the common input of 100 fixed-dt steps.  Wave speeds inflated by
-    k = 1.2: with k = 1 the HLL run loses positivity at t = 0.1375 on this
-    grid, in the oracle itself (R14)."""
+    128^2 grid, then used as the common input of both sides.  Wave speeds inflated by k = 1.2
+    (PAPER.md L409, L416): with k = 1 the HLL run loses positivity at t = 0.1375 on this grid, in
+    the oracle itself (R14).
+    On this state the scheme amplifies round-off strongly (cells at the jet edges next to the
+    inflow wall sit at sigma_bar = sigma_lim, closure terms ~ 1/sigma_bar^2): two ORACLE runs whose
+    inputs differ by 1e-15 relative differ by ~1e-11 after ONE step and by ~1e-3 after 100
+    (R24).  So the bar is condition-aware: the GPU may differ from the oracle by no more
+    than 10x what a 1e-15 perturbation of the input does to the oracle itself (and never needs to
+    beat 1e-10); over 100 steps the density field and the conserved totals are compared too."""
     prob = wl.crossed_jets(128, Kn=1.0, ws_scale=1.2)
     so = oracle_solver(mmo, prob)
     so.advance_to(0.15, 0.4)
     U0 = so.get_state()
+    rng = np.random.default_rng(1)
+    U1 = U0 * (1.0 + 1e-15 * rng.integers(-2, 3, size=U0.shape))
     dt = 0.5 * scout_dt(mmo, prob, 100, 0.4, U0)
     sg = mm.Solver.from_problem(prob, load_state=False)
-    sg.set_state(U0)
-    so.set_state(U0)
-    so.step_fixed_dt(100, dt); sg.step_fixed_dt(100, dt)
-    assert_parity(sg.get_state(), so.get_state())
-    # CFL stepping from the same state: same number of steps to the same time
+    sp = oracle_solver(mmo, prob)                      # the perturbed oracle run
+    sg.set_state(U0); so.set_state(U0); sp.set_state(U1)
+    done = 0
+    for nsteps in (5, 100):
+        so.step_fixed_dt(nsteps - done, dt); sp.step_fixed_dt(nsteps - done, dt)
+        sg.step_fixed_dt(nsteps - done, dt)
+        done = nsteps
+        Ug, Uo, Up = sg.get_state(), so.get_state(), sp.get_state()
+        sens = rel_err(Up, Uo).max()
+        assert_parity(Ug, Uo, max(TOL, 10.0 * sens))
+        rho_noise = np.abs(Up[0] - Uo[0]).mean()
+        assert np.abs(Ug[0] - Uo[0]).mean() <= 10.0 * rho_noise + 1e-13 * np.abs(Uo[0]).mean()
+    # CFL stepping from the same state: same number of steps to (nearly) the same time
     so.set_state(U0); sg.set_state(U0)
-    so.step(20, 0.4); sg.step(20, 0.4)
+    so.step(5, 0.4); sg.step(5, 0.4)
     assert sg.info()["t"] == pytest.approx(so.info()["t"], rel=1e-9)
-    assert_parity(sg.get_state(), so.get_state(), 1e-8)
+    sp.set_state(U1); sp.step(5, 0.4)
+    assert_parity(sg.get_state(), so.get_state(), max(1e-9, 10.0 * rel_err(sp.get_state(), so.get_state()).max()))
 
 
 def test_C4_jets_2048_sampled_windows(mm, mmo):
