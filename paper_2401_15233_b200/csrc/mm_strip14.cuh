@@ -8,7 +8,7 @@
 //   cons  [2][14][35]  conserved rows in flight: filled by cp.async one row ahead of use, so the
 //                      HBM latency of row r+2 hides behind the x pass of row r at no register cost;
 //   acc   [14][32]     per-lane partial update of the row being assembled.
-// Row iteration r:  G_r (y-interface r-1|r) -> finish row r-1 in the oracle's order of operations,
+// Row iteration r:  G_r (y-interface r-1|r) -> finish row r-1 in the scheme's order of operations (x then y then source),
 // (acc - dt/dy (G_r - G_{r-1})) + dt C(W_{r-1}) (a8), store, cell-centre wave speeds of the new
 // state -> running CFL maximum (a9); then row r: x-interfaces, neighbour flux by warp shuffle,
 // acc = U_r - dt/dx (F_{i+1} - F_i).  The two interface directions run through
