@@ -35,13 +35,13 @@ UNIT = "cell-updates/s"
 CFL = 0.4
 
 
-def flops_per_cell_update(shared_limiter: bool):
+def flops_per_cell_update(shared_limiter: bool, zsym: bool):
     """Algorithmic FP64 operations per cell update (each + - * / sqrt exp log = 1).
     -> (count of the formulation the CUDA path runs, count of the oracle's naive restatement).
     The roofline line uses the FIRST (smaller) number: flops the kernel does not execute are not
     credited to it.  Both are produced by committed counting builds, not typed in."""
     from paper_2401_15233_b200 import build_ext
-    k = build_ext.read_opcount()["kernel_flops_per_cell_update_14_"
+    k = build_ext.read_opcount()["kernel_flops_per_cell_update_14_" + ("zsym_" if zsym else "")
                                  + ("shared_limiter" if shared_limiter else "per_variable_limiter")]
     o = None
     for line in (ROOT / "tests" / "golden" / "oracle_opcount.txt").read_text().splitlines():
@@ -168,6 +168,8 @@ def run_gpu(args):
     U_host = torch.empty((14, n, n), dtype=torch.float64).pin_memory()
     W_dev = W_host.to(f"cuda:{local}")
 
+    if args.general_path:
+        s.set_fast_path(False)
     # ---- device-resident timing: K steps, inputs in HBM (two 470 MB copies >> 126 MB L2)
     s.set_state_prim(W_dev)
     s.step(W, CFL)
@@ -209,7 +211,7 @@ def run_gpu(args):
     finite = bool(torch.isfinite(U_host).all())
 
     if rank == 0:
-        fpc, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]))
+        fpc, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]), s.fast_path_active)
         peak_tf = mm.mm_measure_fp64_peak(5)
         kern_avg_ms = kern_ms / max(kern_n, 1)
         achieved_tf = fpc * cells / (kern_avg_ms * 1e-3) * 1e-12
@@ -238,7 +240,8 @@ def run_gpu(args):
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved_tf / peak_tf if peak_tf else None, "traffic": None,
-                         "kernel": "k_step14", "kernel_ms": kern_avg_ms,
+                         "kernel": "k_step14_strip<zsym>" if s.fast_path_active else "k_step14_strip<general>",
+                         "kernel_ms": kern_avg_ms,
                          "flops_per_cell_update": fpc, "flops_per_cell_update_oracle": fpc_oracle,
                          "peak_source": "FP64 DFMA loop measured in this run (mm_measure_fp64_peak)",
                          "hbm_algorithmic_gbs": hbm_gbs, "hbm_peak_gbs": pk.get("hbm_gbs"),
@@ -261,6 +264,8 @@ def main():
     ap.add_argument("--ref-n", type=int, default=256, help="grid of the bounded oracle sample")
     ap.add_argument("--cpu-steps", type=int, default=40)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--general-path", action="store_true",
+                    help="forbid the z-symmetric kernel variant (measurement of the general one)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -117,6 +117,16 @@ int mm_cfl_dt(mm_solver *s, double cfl, double *dt);
 /* Number of kernel launches enqueued by this solver so far. */
 long long mm_launch_count(const mm_solver *s);
 
+/* z-symmetric fast path (SURVEY.md section 8(a) design note).  When the
+ * state given to mm_set_state* and every Dirichlet boundary state have
+ * u_z = P_xz = P_yz = q_z = 0 exactly (checked on the device at mm_set_state*), the scheme keeps
+ * them zero for all time and the 14-moment step runs a kernel variant in which they are
+ * compile-time zeros; all 14 arrays are still carried and written.  The general variant runs
+ * otherwise.  mm_set_fast_path(s, 0) forces the general variant (default: allowed = 1);
+ * mm_fast_path_active returns 1 when the next mm_step* would run the fast variant. */
+int mm_set_fast_path(mm_solver *s, int allow);
+int mm_fast_path_active(const mm_solver *s);
+
 /* Measurement hooks (used by bench.py for the roofline line).
  * Between mm_profile_begin and mm_profile_end every launch of the fused step kernel is
  * bracketed by CUDA events on the solver's stream; mm_profile_end synchronises and returns the
@@ -127,6 +137,10 @@ int mm_profile_end(mm_solver *s, double *step_kernel_ms, long long *launches);
  * `stream` (cudaStream_t): 2 flop per FMA, best of `repeats` launches.  This is the roofline
  * denominator of this FP64-ALU-bound method; MEASURED_PEAKS.json has no FP64 entry. */
 int mm_measure_fp64_peak(void *stream, int repeats, double *tflops);
+/* Accuracy of the library's branch-free reciprocal and square root (Newton on the hardware
+ * seeds) against IEEE division / sqrt over n pseudo-random normal arguments spanning
+ * 1e-30 .. 1e30 on `stream`: max relative error of each, in units of 2^-53. */
+int mm_selftest_fastmath(void *stream, int n, double *max_ulp_rcp, double *max_ulp_sqrt);
 
 void mm_destroy(mm_solver *s);
 const char *mm_strerror(int status);

@@ -116,9 +116,11 @@ def crossed_jets(n: int = 512, Kn: float = 1.0, perturb: float = 0.0, mach: floa
 
 
 def random_smooth14(nx: int, ny: int, seed: int = SEED, amp: float = 0.2, periodic: bool = True,
-                    Kn=None, **options):
+                    Kn=None, zsym: bool = False, **options):
     """Generic smooth, fully 3-D non-equilibrium test state on a periodic box: every one of the
-    14 primitives varies (including the z-odd ones) so no component of the scheme is idle."""
+    14 primitives varies (including the z-odd ones) so no component of the scheme is idle.
+    zsym=True sets the z-odd primitives u_z, P_xz, P_yz, q_z to exactly zero (the symmetry every
+    BASELINE config has) and leaves the other ten as they are."""
     x = (np.arange(nx) + 0.5) / nx
     y = (np.arange(ny) + 0.5) / ny
     X, Y = np.meshgrid(x, y)
@@ -140,6 +142,8 @@ def random_smooth14(nx: int, ny: int, seed: int = SEED, amp: float = 0.2, period
     c3 = rho * (Ph / rho) ** 1.5
     W0[10] = 0.3 * amp * c3 * wave(33); W0[11] = 0.3 * amp * c3 * wave(36); W0[12] = 0.3 * amp * c3 * wave(39)
     W0[13] = 15.0 * Ph * Ph / rho * (1.0 + 0.3 * amp * wave(42))
+    if zsym:
+        W0[3] = 0.0; W0[6] = 0.0; W0[8] = 0.0; W0[12] = 0.0
     t = BC_PERIODIC if periodic else BC_TRANSMISSIVE
     bcs = [dict(type=t)] * 4
     col = dict(model=TAU_KN, Kn=Kn, L_ref=1.0, rho_ref=1.0) if Kn is not None else dict(model=TAU_NONE)

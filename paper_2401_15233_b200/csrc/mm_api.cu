@@ -16,6 +16,12 @@ namespace {
 constexpr int kNT5 = 128;               // 5-moment cells per block
 constexpr int kRateNT = 256;
 
+// resident blocks per SM the two step-kernel variants are compiled for (shared memory bound)
+constexpr size_t kSmemGen = (size_t)kStripWPB * Mom<false>::warp_smem_doubles * sizeof(double);
+constexpr size_t kSmemZS = (size_t)kStripWPB * Mom<true>::warp_smem_doubles * sizeof(double);
+constexpr int kMinBlocksGen = (int)((227 * 1024) / (kSmemGen + 1024));
+constexpr int kMinBlocksZS = (int)((227 * 1024) / (kSmemZS + 1024));
+
 thread_local char g_cuda_msg[256] = "";
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -45,7 +51,7 @@ bool make_layout(const mm_grid* g, Layout* L)
     return true;
 }
 
-// Strips are 31 cells wide; rows are cut into nchunks chunks so that the nstrips * nchunks warp
+// Strips are kSW cells wide; rows are cut into nchunks chunks so that the nstrips * nchunks warp
 // items fill whole waves of the `slots` resident warps.  A chunk of n rows costs n + ~0.8 row
 // passes (one extra y-interface row and three extra row conversions).
 void choose_decomposition(int nx, int ny, int slots, int* nstrips, int* nchunks)
@@ -77,8 +83,10 @@ struct mm_solver {
     int slot;           // accumulator slot holding the current state's CFL reduction
     int has_state;
     long long launches;
-    size_t smem14;
-    int nstrips, nchunks;   // 14-moment work decomposition (mm_strip14.cuh)
+    int nstrips, nchunks[2];   // 14-moment work decomposition (mm_strip14.cuh): [general, z-symmetric]
+    int zsym;               // state and boundary data have no z-odd moment: fast path applies
+    int allow_fast;         // mm_set_fast_path
+    int sms;
     bool profiling;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the step kernel while profiling
 };
@@ -123,10 +131,16 @@ int launch_step(mm_solver* s, const StepCtl& sc)
         MM_LAUNCHED(s, "k_step5");
     } else {
         if ((rc = launch_ghost<14>(s, sc, 1))) return rc;
-        const int items = s->nstrips * s->nchunks;
+        const int fast = s->zsym && s->allow_fast;
+        const int items = s->nstrips * s->nchunks[fast];
+        const int nb = (items + kStripWPB - 1) / kStripWPB;
         if (e0) MM_CUDA(cudaEventRecord(e0, s->stream));
-        k_step14_strip<<<(items + kStripWPB - 1) / kStripWPB, 32 * kStripWPB, s->smem14, s->stream>>>(
-            s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks);
+        if (fast)
+            k_step14_strip<true, kMinBlocksZS><<<nb, 32 * kStripWPB, kSmemZS, s->stream>>>(
+                s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks[1]);
+        else
+            k_step14_strip<false, kMinBlocksGen><<<nb, 32 * kStripWPB, kSmemGen, s->stream>>>(
+                s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks[0]);
         MM_LAUNCHED(s, "k_step14_strip");
     }
     if (e1) MM_CUDA(cudaEventRecord(e1, s->stream));
@@ -170,6 +184,11 @@ int set_state_impl(mm_solver* s, const double* src, int on_device, bool prim)
     k_rate<NM, kRateNT><<<nb, kRateNT, 0, s->stream>>>(s->p, s->U[s->cur], s->ctrl, 0);
     MM_LAUNCHED(s, "k_rate");
     s->has_state = 1;
+    if constexpr (NM == 14) {        // fast-path precondition, checked on the device by k_rate / k_bc_table
+        Ctrl h;
+        if ((rc = read_ctrl(s, &h))) return rc;
+        s->zsym = !h.znz && !h.bc_znz;
+    }
     return MM_OK;
 }
 
@@ -276,14 +295,18 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
     delete hb;
     if (e != cudaSuccess) { delete s; return cuda_fail(e, "mm_create workspace init"); }
 
-    s->smem14 = (size_t)kStripWPB * kWarpSmemD * sizeof(double);
+    s->allow_fast = 1;
     if (nm == 14) {
-        e = cudaFuncSetAttribute(k_step14_strip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->smem14);
+        e = cudaFuncSetAttribute(k_step14_strip<false, kMinBlocksGen>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_step14_strip<true, kMinBlocksZS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
         if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaFuncSetAttribute(k_step14_strip)"); }
         int dev = 0, sms = 148;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        choose_decomposition(grid->nx, grid->ny, sms * 8, &s->nstrips, &s->nchunks);
+        s->sms = sms;
+        choose_decomposition(grid->nx, grid->ny, sms * kMinBlocksGen * kStripWPB, &s->nstrips, &s->nchunks[0]);
+        choose_decomposition(grid->nx, grid->ny, sms * kMinBlocksZS * kStripWPB, &s->nstrips, &s->nchunks[1]);
         k_bc_table<14><<<4, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 4);
     } else {
         k_bc_table<5><<<2, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 2);
@@ -391,6 +414,15 @@ int mm_cfl_dt(mm_solver* s, double cfl, double* dt)
 
 long long mm_launch_count(const mm_solver* s) { return s ? s->launches : 0; }
 
+int mm_set_fast_path(mm_solver* s, int allow)
+{
+    if (!s) return MM_EINVAL;
+    s->allow_fast = allow ? 1 : 0;
+    return MM_OK;
+}
+
+int mm_fast_path_active(const mm_solver* s) { return s ? (s->zsym && s->allow_fast && s->L.nm == 14) : 0; }
+
 int mm_profile_begin(mm_solver* s)
 {
     if (!s) return MM_EINVAL;
@@ -445,6 +477,23 @@ int mm_measure_fp64_peak(void* stream, int repeats, double* tflops)
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
     *tflops = best;
+    return MM_OK;
+}
+
+int mm_selftest_fastmath(void* stream, int n, double* max_ulp_rcp, double* max_ulp_sqrt)
+{
+    if (n < 1 || !max_ulp_rcp || !max_ulp_sqrt) return MM_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* d = nullptr;
+    MM_CUDA(cudaMalloc(&d, 2 * sizeof(unsigned long long)));   // measurement scratch only
+    cudaMemsetAsync(d, 0, 2 * sizeof(unsigned long long), st);
+    k_fastmath_test<<<296, 256, 0, st>>>(n, d, d + 1);
+    unsigned long long h[2] = {0, 0};
+    cudaError_t e = cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "k_fastmath_test");
+    *max_ulp_rcp = bits2d(h[0]); *max_ulp_sqrt = bits2d(h[1]);
     return MM_OK;
 }
 

@@ -18,10 +18,12 @@ struct Ctrl {
     unsigned long long rate_bits[2], speed_bits[2];   // max-reduced as ordered bit patterns (>= 0)
     double ghost_rate, ghost_speed;                   // constant part from Dirichlet ghost states
     long long bc_bad;                                 // a Dirichlet state has rho <= 0 or P <= 0
+    long long bc_znz;                                 // a Dirichlet state has a non-zero z-odd moment
     long long steps;
     int bad[2];                                       // reduction saw rho<=0, P<=0 or non-finite
     int failed;                                       // sticky: stepping stopped (MM_ENONFINITE)
     int skip;                                         // this step leaves the state untouched
+    int znz;                                          // the state set by mm_set_state has a non-zero z-odd moment
 };
 
 // Boundary tables (device memory): conserved ghost states of the Dirichlet sides.
@@ -74,7 +76,7 @@ __device__ __forceinline__ void block_reduce_rate(double rate, double speed, int
 }
 
 // rate / speed / validity of one cell from its conserved moments
-template <int NM>
+template <int NM, class Z = double>
 __device__ __forceinline__ void cell_rate(const Params& p, const double (&U)[NM], double& rate,
                                           double& speed, int& bad)
 {
@@ -86,9 +88,9 @@ __device__ __forceinline__ void cell_rate(const Params& p, const double (&U)[NM]
         ok = cell_speed5(p, W, sx);
         rate = sx / p.dx; speed = sx;
     } else {
-        cons2prim14(U, W);
+        cons2prim14<Z>(U, W);
         double sx, sy;
-        ok = cell_speeds14(p, W, sx, sy);
+        ok = cell_speeds14<Z>(p, W, sx, sy);
         rate = fmax(sx / p.dx, sy / p.dy); speed = fmax(sx, sy);
     }
     // finite test: NaN or Inf fail (x - x != 0)
@@ -107,7 +109,7 @@ __global__ void k_pack(Params p, const double* __restrict__ src, double* __restr
 #pragma unroll
     for (int m = 0; m < NM; ++m) a[m] = src[m * n + (size_t)j * p.nx + i];
     if constexpr (PRIM) {
-        if constexpr (NM == 5) prim2cons5(a, b); else prim2cons14(a, b);
+        if constexpr (NM == 5) prim2cons5(a, b); else prim2cons14<double>(a, b);
     } else {
 #pragma unroll
         for (int m = 0; m < NM; ++m) b[m] = a[m];
@@ -126,7 +128,7 @@ __global__ void k_unpack(Params p, const double* __restrict__ src, double* __res
 #pragma unroll
     for (int m = 0; m < NM; ++m) a[m] = src[m * plane + (size_t)(j + 2) * p.pitch + i + 2];
     if constexpr (PRIM) {
-        if constexpr (NM == 5) cons2prim5(a, b); else cons2prim14(a, b);
+        if constexpr (NM == 5) cons2prim5(a, b); else cons2prim14<double>(a, b);
     } else {
 #pragma unroll
         for (int m = 0; m < NM; ++m) b[m] = a[m];
@@ -149,7 +151,7 @@ __global__ void k_bc_table(Params p, BcTable* tab, Ctrl* ctrl, int nsides)
     double W[NM], U[NM];
 #pragma unroll
     for (int m = 0; m < NM; ++m) W[m] = b.W[k][m];
-    if constexpr (NM == 5) prim2cons5(W, U); else prim2cons14(W, U);
+    if constexpr (NM == 5) prim2cons5(W, U); else prim2cons14<double>(W, U);
 #pragma unroll
     for (int m = 0; m < NM; ++m) b.U[k][m] = U[m];
     double rate, speed; int bad = 0;
@@ -158,6 +160,9 @@ __global__ void k_bc_table(Params p, BcTable* tab, Ctrl* ctrl, int nsides)
     atomic_max_pos(reinterpret_cast<unsigned long long*>(&ctrl->ghost_rate), rate);
     atomic_max_pos(reinterpret_cast<unsigned long long*>(&ctrl->ghost_speed), speed);
     if (bad) ctrl->bc_bad = 1;
+    if constexpr (NM == 14) {
+        if (W[3] != 0.0 || W[6] != 0.0 || W[8] != 0.0 || W[12] != 0.0) ctrl->bc_znz = 1;
+    }
 }
 
 // ------------------------------------------------------------------- ghost cells (L426)
@@ -239,7 +244,7 @@ __global__ void __launch_bounds__(NT) k_rate(Params p, const double* __restrict_
 {
     const size_t plane = (size_t)p.rows * p.pitch;
     double rate = 0.0, speed = 0.0;
-    int bad = 0;
+    int bad = 0, znz = 0;
     const long long n = (long long)p.nx * p.ny;
     for (long long c = (long long)blockIdx.x * NT + threadIdx.x; c < n; c += (long long)gridDim.x * NT) {
         const int i = (int)(c % p.nx), j = (int)(c / p.nx);
@@ -249,147 +254,59 @@ __global__ void __launch_bounds__(NT) k_rate(Params p, const double* __restrict_
         double r, s;
         cell_rate<NM>(p, u, r, s, bad);
         rate = fmax(rate, r); speed = fmax(speed, s);
+        if constexpr (NM == 14) {
+            if (u[3] != 0.0 || u[6] != 0.0 || u[8] != 0.0 || u[12] != 0.0) znz = 1;
+        }
     }
+    if (__syncthreads_or(znz) && threadIdx.x == 0) ctrl->znz = 1;
     block_reduce_rate<NT>(rate, speed, bad, ctrl, slot);
 }
 
 // ------------------------------------------------------------------ the fused time step
-// Interface flux between cell a (low side) and cell b (high side) along one direction, from the
-// primitives staged in shared memory.  `w` points at cell b of moment plane 0, `cs` is the cell
-// stride along the direction, `ms` the plane stride.  MUSCL on primitives (L262-264): face
-// states W_a + slope_a/2 and W_b - slope_b/2; closure flux, conserved state and wave speeds of
-// both (eval_face*), then HLL / Rusanov.  For the y direction (SWAP) the state is index-swapped
-// on load and the flux swapped back on return (L414).
-template <int NM, bool SWAP>
-__device__ __forceinline__ void interface_flux(const Params& p, const double* __restrict__ w,
-                                               int cs, int ms, double (&Fh)[NM])
+// (the 14-moment step kernel is in mm_strip14.cuh)
+// 5-moment interface flux between cell a (low side) and cell b (high side) from the primitives
+// staged in shared memory.  `w` points at cell b of moment plane 0, `ms` is the plane stride.
+// MUSCL on primitives (L262-264): face states W_a + slope_a/2 and W_b - slope_b/2; closure flux,
+// conserved state and wave speeds of both (eval_face5), then HLL / Rusanov.
+__device__ __forceinline__ void interface_flux5(const Params& p, const double* __restrict__ w,
+                                                int ms, double (&Fh)[5])
 {
-    double WL[NM], WR[NM];
+    constexpr int NM = 5;
+    double Wam[NM], Wa[NM], Wb[NM], Wbp[NM], WL[NM], WR[NM];
+#pragma unroll
+    for (int k = 0; k < NM; ++k) {
+        const double* q = w + k * ms;
+        Wam[k] = q[-2]; Wa[k] = q[-1]; Wb[k] = q[0]; Wbp[k] = q[1];
+    }
     if (p.limiter != 0 && p.shared_limiter) {
-        double Wam[NM], Wa[NM], Wb[NM], Wbp[NM], ha[NM], hb[NM];
+        PsiMin ma, mb;
 #pragma unroll
         for (int k = 0; k < NM; ++k) {
-            const double* q = w + (SWAP ? swap_xy(k) : k) * ms;
-            Wam[k] = q[-2 * cs]; Wa[k] = q[-cs]; Wb[k] = q[0]; Wbp[k] = q[cs];
+            ma.add(p.limiter, Wa[k] - Wam[k], Wb[k] - Wa[k]);
+            mb.add(p.limiter, Wb[k] - Wa[k], Wbp[k] - Wb[k]);
         }
-        half_slopes<NM>(p, Wam, Wa, Wb, ha);
-        half_slopes<NM>(p, Wa, Wb, Wbp, hb);
+        const double qa = 0.25 * ma.psi(), qb = 0.25 * mb.psi();
 #pragma unroll
-        for (int k = 0; k < NM; ++k) { WL[k] = Wa[k] + ha[k]; WR[k] = Wb[k] - hb[k]; }
+        for (int k = 0; k < NM; ++k) {
+            WL[k] = Wa[k] + qa * ((Wa[k] - Wam[k]) + (Wb[k] - Wa[k]));
+            WR[k] = Wb[k] - qb * ((Wb[k] - Wa[k]) + (Wbp[k] - Wb[k]));
+        }
     } else {
 #pragma unroll
         for (int k = 0; k < NM; ++k) {
-            const double* q = w + (SWAP ? swap_xy(k) : k) * ms;
-            const double am = q[-2 * cs], a = q[-cs], b = q[0], bp = q[cs];
             double ha = 0.0, hb = 0.0;
             if (p.limiter != 0) {
-                const double d = b - a;
-                ha = 0.5 * limited_slope(p.limiter, a - am, d);
-                hb = 0.5 * limited_slope(p.limiter, d, bp - b);
+                const double d = Wb[k] - Wa[k];
+                ha = 0.5 * limited_slope(p.limiter, Wa[k] - Wam[k], d);
+                hb = 0.5 * limited_slope(p.limiter, d, Wbp[k] - Wb[k]);
             }
-            WL[k] = a + ha; WR[k] = b - hb;
+            WL[k] = Wa[k] + ha; WR[k] = Wb[k] - hb;
         }
     }
     double FL[NM], UL[NM], FR[NM], UR[NM], lminL, lmaxL, lminR, lmaxR;
-    if constexpr (NM == 5) {
-        eval_face5(p, WL, FL, UL, lminL, lmaxL);
-        eval_face5(p, WR, FR, UR, lminR, lmaxR);
-    } else {
-        eval_face14(p, WL, FL, UL, lminL, lmaxL);
-        eval_face14(p, WR, FR, UR, lminR, lmaxR);
-    }
+    eval_face5(p, WL, FL, UL, lminL, lmaxL);
+    eval_face5(p, WR, FR, UR, lminR, lmaxR);
     numflux<NM>(p.flux, FL, FR, UL, UR, lminL, lmaxL, lminR, lmaxR, Fh);
-}
-
-// 14-moment 2-D step.  One block = one TX x TY tile of cells:
-//   1. stage the tile + 2-cell halo of the conserved moments in shared memory and convert to
-//      primitives in place (a2);
-//   2. x pass: the (TX+1) x TY x-interfaces of the tile -> Fx (a3-a7);
-//   3. y pass: the TX x (TY+1) y-interfaces -> Fy;
-//   4. one thread per cell: U^{n+1} = U^n - dt/dx dFx - dt/dy dFy + dt C(W^n) (a8), store, then
-//      the wave speeds of the NEW cell state feed the CFL max-reduction for the next dt (a9).
-template <int TX, int TY>
-__global__ void __launch_bounds__(TX * TY)
-k_step14(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl, int slot_next)
-{
-    constexpr int NM = 14, NT = TX * TY, TXH = TX + 4, TYH = TY + 4;
-    constexpr int PW = TYH * TXH, PFX = TY * (TX + 1), PFY = (TY + 1) * TX;
-    extern __shared__ double smem[];
-    double* Ws = smem;                 // [14][TYH][TXH]
-    double* Fx = Ws + NM * PW;         // [14][TY][TX+1]
-    double* Fy = Fx + NM * PFX;        // [14][TY+1][TX]
-    const int tid = threadIdx.x;
-    const int gx0 = blockIdx.x * TX, gy0 = blockIdx.y * TY;
-    const size_t plane = (size_t)p.rows * p.pitch;
-    const double dt = ctrl->dt;
-    const int ci = tid % TX, cj = tid / TX;
-    const bool cell_ok = gx0 + ci < p.nx && gy0 + cj < p.ny;
-    const size_t cidx = (size_t)(gy0 + cj + 2) * p.pitch + gx0 + ci + 2;
-
-    if (ctrl->skip) {                  // failed / past t_end: carry the state over unchanged
-        if (cell_ok)
-#pragma unroll
-            for (int m = 0; m < NM; ++m) Uout[m * plane + cidx] = Uin[m * plane + cidx];
-        return;
-    }
-
-    // 1. stage + cons -> prim.  Tile-corner halo cells are in no stencil: skipped.
-    for (int idx = tid; idx < PW; idx += NT) {
-        const int ly = idx / TXH, lx = idx - ly * TXH;
-        const bool corner = (lx < 2 || lx >= TX + 2) && (ly < 2 || ly >= TY + 2);
-        const int px = gx0 + lx, py = gy0 + ly;        // padded coordinates
-        if (corner || px >= p.nx + 4 || py >= p.ny + 4) continue;
-        double U[NM], W[NM];
-        const double* src = Uin + (size_t)py * p.pitch + px;
-#pragma unroll
-        for (int m = 0; m < NM; ++m) U[m] = src[m * plane];
-        cons2prim14(U, W);
-#pragma unroll
-        for (int m = 0; m < NM; ++m) Ws[m * PW + idx] = W[m];
-    }
-    __syncthreads();
-
-    // 2. x interfaces: interface i of row j lies between tile cells i-1 and i
-    for (int idx = tid; idx < PFX; idx += NT) {
-        const int j = idx / (TX + 1), i = idx - j * (TX + 1);
-        if (gx0 + i > p.nx || gy0 + j >= p.ny) continue;
-        double Fh[NM];
-        interface_flux<NM, false>(p, Ws + (j + 2) * TXH + (i + 2), 1, PW, Fh);
-#pragma unroll
-        for (int m = 0; m < NM; ++m) Fx[m * PFX + idx] = Fh[m];
-    }
-    // 3. y interfaces: interface j of column i lies between tile cells j-1 and j
-    for (int idx = tid; idx < PFY; idx += NT) {
-        const int j = idx / TX, i = idx - j * TX;
-        if (gx0 + i >= p.nx || gy0 + j > p.ny) continue;
-        double Fh[NM];
-        interface_flux<NM, true>(p, Ws + (j + 2) * TXH + (i + 2), TXH, PW, Fh);
-#pragma unroll
-        for (int m = 0; m < NM; ++m) Fy[swap_xy(m) * PFY + idx] = Fh[m];
-    }
-    __syncthreads();
-
-    // 4. update + source + tail reduction
-    double rate = 0.0, speed = 0.0;
-    int bad = 0;
-    if (cell_ok) {
-        const double dtdx = dt / p.dx, dtdy = dt / p.dy;
-        double Un[NM], W[NM];
-#pragma unroll
-        for (int m = 0; m < NM; ++m) {
-            const double* fx = Fx + m * PFX + cj * (TX + 1) + ci;
-            const double* fy = Fy + m * PFY + cj * TX + ci;
-            double v = Uin[m * plane + cidx] - dtdx * (fx[1] - fx[0]);
-            Un[m] = v - dtdy * (fy[TX] - fy[0]);
-            W[m] = Ws[m * PW + (cj + 2) * TXH + ci + 2];
-        }
-        if (p.tau_model != 0)
-            add_source14(W, dt * inv_tau(p, W[0], (W[4] + W[7] + W[9]) / 3.0), Un);
-#pragma unroll
-        for (int m = 0; m < NM; ++m) Uout[m * plane + cidx] = Un[m];
-        cell_rate<NM>(p, Un, rate, speed, bad);
-    }
-    block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
 }
 
 // 5-moment 1-D step: one block = NT consecutive cells, same four stages.
@@ -425,7 +342,7 @@ k_step5(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctr
     for (int idx = tid; idx < PF; idx += NT) {
         if (gx0 + idx > p.nx) continue;
         double Fh[NM];
-        interface_flux<NM, false>(p, Ws + idx + 2, 1, PW, Fh);
+        interface_flux5(p, Ws + idx + 2, PW, Fh);
 #pragma unroll
         for (int m = 0; m < NM; ++m) Fx[m * PF + idx] = Fh[m];
     }
@@ -462,6 +379,25 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, doubl
 #pragma unroll
     for (int k = 0; k < 16; ++k) s += x[k];
     if (s == 123.456) out[0] = s;       // never true: keeps the loop alive
+}
+
+
+// max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x)
+__global__ void k_fastmath_test(int n, unsigned long long* err_rcp_bits, unsigned long long* err_sqrt_bits)
+{
+    double er = 0.0, es = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        unsigned long long z = (unsigned long long)i * 0x9E3779B97F4A7C15ull + 0x2401152330ull;
+        z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
+        const double m = 1.0 + (double)(z >> 11) * (1.0 / 9007199254740992.0);       // [1, 2)
+        const double x = m * exp2((double)((int)(z & 255) - 128) * 0.78);            // ~1e-30 .. 1e30
+        const double r0 = 1.0 / x, s0 = sqrt(x);
+        er = fmax(er, fabs(rcp(x) - r0) / r0);
+        es = fmax(es, fabs(fsqrt(x) - s0) / s0);
+    }
+    const double ulp = 1.1102230246251565e-16;
+    atomic_max_pos(err_rcp_bits, er / ulp);
+    atomic_max_pos(err_sqrt_bits, es / ulp);
 }
 
 }  // namespace mm

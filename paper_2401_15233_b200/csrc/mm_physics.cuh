@@ -4,13 +4,83 @@
 // kept as 6 scalars, the closure is only evaluated for the components the x-flux needs, and
 // powers of the pressure tensor use the Cayley-Hamilton identity instead of matrix products.
 // The y direction reuses the x routines on index-swapped states (L414).
+//
+// The 14-moment routines are templates over the type Z of the z-odd quantities
+// (u_z, P_xz, P_yz, q_z and everything derived from them): Z = double is the general path;
+// Z = zero_t is the z-symmetric fast path, in which those quantities are exact compile-time
+// zeros and every product with them disappears from the instruction stream.  It is selected
+// only when the state and the boundary data have u_z = P_xz = P_yz = q_z = 0 exactly
+// (checked on the device at mm_set_state); such a state keeps them zero for all time.
 #pragma once
 #ifndef MM_OPCOUNT_HOST          // csrc/opcount_host.cpp compiles this header on the host instead
 #include <cuda_runtime.h>
 #include <math.h>
 #endif
+#include <type_traits>
 
 namespace mm {
+
+// ------------------------------------------------------------------ exact compile-time zero
+struct zero_t {};
+template <class T> __host__ __device__ __forceinline__ zero_t operator*(zero_t, const T&) { return {}; }
+template <class T> __host__ __device__ __forceinline__ zero_t operator*(const T&, zero_t) { return {}; }
+__host__ __device__ __forceinline__ zero_t operator*(zero_t, zero_t) { return {}; }
+template <class T> __host__ __device__ __forceinline__ T operator+(zero_t, const T& b) { return b; }
+template <class T> __host__ __device__ __forceinline__ T operator+(const T& a, zero_t) { return a; }
+__host__ __device__ __forceinline__ zero_t operator+(zero_t, zero_t) { return {}; }
+template <class T> __host__ __device__ __forceinline__ T operator-(zero_t, const T& b) { return -b; }
+template <class T> __host__ __device__ __forceinline__ T operator-(const T& a, zero_t) { return a; }
+__host__ __device__ __forceinline__ zero_t operator-(zero_t, zero_t) { return {}; }
+__host__ __device__ __forceinline__ zero_t operator-(zero_t) { return {}; }
+
+// read / write a z-odd slot of a 14-array: nothing is touched on the zero path
+template <class Z> __host__ __device__ __forceinline__ Z zget(const double& x)
+{
+    if constexpr (std::is_same<Z, zero_t>::value) return zero_t{}; else return x;
+}
+__host__ __device__ __forceinline__ void zput(double& dst, const double& v) { dst = v; }
+__host__ __device__ __forceinline__ void zput(double&, zero_t) {}
+__host__ __device__ __forceinline__ void zadd(double& dst, const double& v) { dst = dst + v; }
+__host__ __device__ __forceinline__ void zadd(double&, zero_t) {}
+
+// ------------------------------------------------------------------ reciprocal / square root
+// rcp(x) ~ 1/x and fsqrt(x) ~ sqrt(x) to ~1 ulp for normal x: hardware seed (MUFU.RCP64H /
+// MUFU.RSQ64H, ~20 bits) + one higher-order Newton step, branch-free (no slow-path call).
+// fsqrt(x) = 0 for |x| < 1e-290; negative or NaN arguments give NaN.  rcp is only applied to
+// well-scaled arguments (densities, pressures, O(1) determinants, wave-speed differences).
+// -DMM_EXACT_MATH restores IEEE div/sqrt.
+#ifdef MM_OPCOUNT_HOST
+__forceinline__ double rcp(double x) { return 1.0 / x; }
+__forceinline__ double fsqrt(double x) { return sqrt(x); }
+#elif defined(MM_EXACT_MATH)
+__device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
+__device__ __forceinline__ double fsqrt(double x) { return sqrt(x); }
+#else
+__device__ __forceinline__ double rcp(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const double e = fma(-x, r, 1.0);          // |e| <~ 2^-20
+    const double e2 = fma(e, e, e);            // e + e^2
+    const double e3 = fma(e2, e, e);           // e + e^2 + e^3
+    return fma(r, e3, r);                      // r (1 + e + e^2 + e^3): error e^4
+}
+__device__ __forceinline__ double fsqrt(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double s0 = x * y;
+    const double e = fma(-s0, y, 1.0);         // 1 - x y^2
+    const double pe = fma(0.375, e, 0.5);
+    const double y1 = fma(y * e, pe, y);       // y (1 + e/2 + 3e^2/8): error ~ e^3
+    double s = x * y1;
+    const double r = fma(-s, s, x);            // final Newton correction of the root itself
+    s = fma(r, 0.5 * y1, s);
+    // the hardware seed flushes subnormal arguments to zero (-> inf): everything below 1e-290
+    // is returned as 0 (absolute error < 1e-145); negative or NaN arguments still give NaN
+    return fabs(x) < 1e-290 ? 0.0 : s;
+}
+#endif
 
 // x <-> y swap of the 14 moments (primitive or conserved); an involution.
 __host__ __device__ constexpr int swap_xy(int m)
@@ -18,6 +88,8 @@ __host__ __device__ constexpr int swap_xy(int m)
     const int t[14] = {0, 2, 1, 3, 7, 5, 8, 4, 6, 9, 11, 10, 12, 13};
     return t[m];
 }
+// z-odd moments: u_z, P_xz, P_yz, q_z (a set closed under swap_xy)
+__host__ __device__ constexpr bool z_odd(int m) { return m == 3 || m == 6 || m == 8 || m == 12; }
 
 struct Params {               // per-solver constants, passed by value to the kernels
     double sigma_lim;         // L163, L512
@@ -36,55 +108,38 @@ __device__ __forceinline__ double clamp_sigma(double s, double lim)
 }
 
 // ------------------------------------------------------------------ limiter (L262-266)
-// psi in [0,1] multiplying the central slope (dm+dp)/2.
-__device__ __forceinline__ double limiter_psi(int lim, double dm, double dp)
-{
-    if (!(dm * dp > 0.0)) return 0.0;
-    if (lim == 1) {
-        double am = fabs(dm), ap = fabs(dp);
-        return 2.0 * fmin(am, ap) / (am + ap);
-    }
-    return 2.0 * dm * dp / (dm * dm + dp * dp);
-}
 // the limited slope itself: minmod(dm,dp) resp. symmetric van Albada dm dp (dm+dp)/(dm^2+dp^2)
 __device__ __forceinline__ double limited_slope(int lim, double dm, double dp)
 {
     if (!(dm * dp > 0.0)) return 0.0;
     if (lim == 1) return fabs(dm) < fabs(dp) ? dm : dp;
-    return dm * dp * (dm + dp) / (dm * dm + dp * dp);
+    return dm * dp * (dm + dp) / (dm * dm + dp * dp);     // IEEE: differences may be subnormal
 }
 
-// Half slopes h[k] = slope_k / 2 of one cell along one direction from its two neighbours.
-template <int NM>
-__device__ __forceinline__ void half_slopes(const Params& p, const double (&Wm)[NM],
-                                            const double (&W0)[NM], const double (&Wp)[NM],
-                                            double (&hs)[NM])
-{
-    if (p.limiter == 0) {
-#pragma unroll
-        for (int k = 0; k < NM; ++k) hs[k] = 0.0;
-        return;
+// Shared, most stringent limiter value (L266) over a set of variables, without a division per
+// variable: psi_k = 2 n_k / d_k with (n_k, d_k) = (min(|dm|,|dp|), |dm|+|dp|) for minmod and
+// (dm dp, dm^2+dp^2) for van Albada when dm dp > 0, psi_k = 0 otherwise; a variable with
+// dm = dp = 0 imposes nothing (R14).  The running minimum is kept as a fraction
+// n/d and compared by cross-multiplication; psi = 2 n / d is formed once at the end.
+struct PsiMin {
+    double n = 0.5, d = 1.0;
+    __device__ __forceinline__ void add(int lim, double dm, double dp)
+    {
+        const double prod = dm * dp;
+        double nk, dk;
+        if (lim == 1) { nk = fmin(fabs(dm), fabs(dp)); dk = fabs(dm) + fabs(dp); }
+        else { nk = prod; dk = dm * dm + dp * dp; }
+        const bool pos = prod > 0.0;
+        const bool flat = (dm == 0.0) && (dp == 0.0);
+        nk = pos ? nk : (flat ? 0.5 : 0.0);
+        dk = pos ? dk : 1.0;
+        if (nk * d < n * dk) { n = nk; d = dk; }
     }
-    if (p.shared_limiter) {
-        // the same, most stringent psi for all primitives (L266); dm = dp = 0 imposes nothing
-        double psi = 1.0;
-#pragma unroll
-        for (int k = 0; k < NM; ++k) {
-            double dm = W0[k] - Wm[k], dp = Wp[k] - W0[k];
-            if (dm == 0.0 && dp == 0.0) continue;
-            psi = fmin(psi, limiter_psi(p.limiter, dm, dp));
-        }
-#pragma unroll
-        for (int k = 0; k < NM; ++k) {
-            double dm = W0[k] - Wm[k], dp = Wp[k] - W0[k];
-            hs[k] = 0.5 * (psi * (0.5 * (dm + dp)));
-        }
-    } else {
-#pragma unroll
-        for (int k = 0; k < NM; ++k)
-            hs[k] = 0.5 * limited_slope(p.limiter, W0[k] - Wm[k], Wp[k] - W0[k]);
-    }
-}
+    // IEEE division (one per slope): psi is then the correctly rounded 2 n_k / d_k of the
+    // winning variable, which keeps the limiter free of extra round-off -- the shared-psi
+    // scheme amplifies round-off in psi by ~1e3 over 30 steps (R24)
+    __device__ __forceinline__ double psi() const { return (2.0 * n) / d; }
+};
 
 // ============================================================================ 5-moment
 // Eq 12 (L129-137).
@@ -177,256 +232,6 @@ __device__ __forceinline__ void add_source5(const double (&W)[5], double dt_over
     Un[3] += dt_over_tau * (-q);
     Un[4] += dt_over_tau * (-(4.0 * u * q + r - 3.0 * P * P / rho));
 }
-
-// =========================================================================== 14-moment
-// Inverse of the conserved forms of Eq 16 (L169-181).
-__device__ __forceinline__ void cons2prim14(const double (&U)[14], double (&W)[14])
-{
-    double rho = U[0], ir = 1.0 / rho;
-    double ux = U[1] * ir, uy = U[2] * ir, uz = U[3] * ir;
-    double Pxx = U[4] - rho * ux * ux, Pxy = U[5] - rho * ux * uy, Pxz = U[6] - rho * ux * uz;
-    double Pyy = U[7] - rho * uy * uy, Pyz = U[8] - rho * uy * uz, Pzz = U[9] - rho * uz * uz;
-    double u2 = ux * ux + uy * uy + uz * uz, trP = Pxx + Pyy + Pzz;
-    double Pux = Pxx * ux + Pxy * uy + Pxz * uz;
-    double Puy = Pxy * ux + Pyy * uy + Pyz * uz;
-    double Puz = Pxz * ux + Pyz * uy + Pzz * uz;
-    double e = rho * u2 + trP;
-    double qx = U[10] - ux * e - 2.0 * Pux;
-    double qy = U[11] - uy * e - 2.0 * Puy;
-    double qz = U[12] - uz * e - 2.0 * Puz;
-    double uPu = ux * Pux + uy * Puy + uz * Puz, uq = ux * qx + uy * qy + uz * qz;
-    double R = U[13] - rho * u2 * u2 - 2.0 * u2 * trP - 4.0 * uPu - 4.0 * uq;
-    W[0] = rho; W[1] = ux; W[2] = uy; W[3] = uz;
-    W[4] = Pxx; W[5] = Pxy; W[6] = Pxz; W[7] = Pyy; W[8] = Pyz; W[9] = Pzz;
-    W[10] = qx; W[11] = qy; W[12] = qz; W[13] = R;
-}
-
-__device__ __forceinline__ void prim2cons14(const double (&W)[14], double (&U)[14])
-{
-    double rho = W[0], ux = W[1], uy = W[2], uz = W[3];
-    double Pxx = W[4], Pxy = W[5], Pxz = W[6], Pyy = W[7], Pyz = W[8], Pzz = W[9];
-    double u2 = ux * ux + uy * uy + uz * uz, trP = Pxx + Pyy + Pzz;
-    double Pux = Pxx * ux + Pxy * uy + Pxz * uz;
-    double Puy = Pxy * ux + Pyy * uy + Pyz * uz;
-    double Puz = Pxz * ux + Pyz * uy + Pzz * uz;
-    double e = rho * u2 + trP;
-    U[0] = rho; U[1] = rho * ux; U[2] = rho * uy; U[3] = rho * uz;
-    U[4] = rho * ux * ux + Pxx; U[5] = rho * ux * uy + Pxy; U[6] = rho * ux * uz + Pxz;
-    U[7] = rho * uy * uy + Pyy; U[8] = rho * uy * uz + Pyz; U[9] = rho * uz * uz + Pzz;
-    U[10] = ux * e + 2.0 * Pux + W[10];
-    U[11] = uy * e + 2.0 * Puy + W[11];
-    U[12] = uz * e + 2.0 * Puz + W[12];
-    double uPu = ux * Pux + uy * Puy + uz * Puz;
-    double uq = ux * W[10] + uy * W[11] + uz * W[12];
-    U[13] = rho * u2 * u2 + 2.0 * u2 * trP + 4.0 * uPu + 4.0 * uq + W[13];
-}
-
-// Dimensionless state (Eq 6 L75-81, rho* = 1): c = sqrt(P/rho), P = P_ii/3, p = P_ij/P (tr p = 3),
-// h = q/(rho c^3), Rs = R/(rho c^4); plus p^2, adj(p), det p, w = p^-1 h, and sigma (Eq 21 L210).
-struct Star14 {
-    double c, Ph;
-    double pxx, pxy, pxz, pyy, pyz, pzz;     // p
-    double sxx, sxy, sxz, syy, syz, szz;     // p^2
-    double t2, I3;                           // tr p^2, det p
-    double hx, hy, hz, wx, wy, wz;           // h, w = p^-1 h
-    double sigma;                            // Eq 21, unlimited
-};
-
-__device__ __forceinline__ void nondim_sigma14(const double (&W)[14], Star14& s)
-{
-    double rho = W[0];
-    double Ph = (W[4] + W[7] + W[9]) / 3.0;
-    double iP = 1.0 / Ph, ir = 1.0 / rho;
-    double c2 = Ph * ir, c = sqrt(c2);
-    s.c = c; s.Ph = Ph;
-    s.pxx = W[4] * iP; s.pxy = W[5] * iP; s.pxz = W[6] * iP;
-    s.pyy = W[7] * iP; s.pyz = W[8] * iP; s.pzz = W[9] * iP;
-    double ih = iP * (c * rho * iP);                       // 1/(rho c^3) = 1/(P c)
-    s.hx = W[10] * ih; s.hy = W[11] * ih; s.hz = W[12] * ih;
-    double Rs = W[13] * rho * iP * iP;                     // R/(rho c^4) = R rho / P^2
-    s.sxx = s.pxx * s.pxx + s.pxy * s.pxy + s.pxz * s.pxz;
-    s.sxy = s.pxx * s.pxy + s.pxy * s.pyy + s.pxz * s.pyz;
-    s.sxz = s.pxx * s.pxz + s.pxy * s.pyz + s.pxz * s.pzz;
-    s.syy = s.pxy * s.pxy + s.pyy * s.pyy + s.pyz * s.pyz;
-    s.syz = s.pxy * s.pxz + s.pyy * s.pyz + s.pyz * s.pzz;
-    s.szz = s.pxz * s.pxz + s.pyz * s.pyz + s.pzz * s.pzz;
-    s.t2 = s.sxx + s.syy + s.szz;
-    // adjugate (cofactors) of p and det p
-    double axx = s.pyy * s.pzz - s.pyz * s.pyz, axy = s.pxz * s.pyz - s.pxy * s.pzz;
-    double axz = s.pxy * s.pyz - s.pxz * s.pyy, ayy = s.pxx * s.pzz - s.pxz * s.pxz;
-    double ayz = s.pxy * s.pxz - s.pxx * s.pyz, azz = s.pxx * s.pyy - s.pxy * s.pxy;
-    s.I3 = s.pxx * axx + s.pxy * axy + s.pxz * axz;
-    double id = 1.0 / s.I3;
-    s.wx = (axx * s.hx + axy * s.hy + axz * s.hz) * id;
-    s.wy = (axy * s.hx + ayy * s.hy + ayz * s.hz) * id;
-    s.wz = (axz * s.hx + ayz * s.hy + azz * s.hz) * id;
-    // Eq 21 with P_ii P_jj = 9: sigma = [b + sqrt(b^2 + 8 t2 X)]/(4 t2), b = 2 t2 + 9 - R*,
-    // X = h.p^-1.h; conjugate form when b < 0 (DESIGN.md R4)
-    double X = s.hx * s.wx + s.hy * s.wy + s.hz * s.wz;
-    double b = 2.0 * s.t2 + 9.0 - Rs;
-    double D = sqrt(b * b + 8.0 * s.t2 * X);
-    s.sigma = b >= 0.0 ? (b + D) / (4.0 * s.t2) : 2.0 * X / (D - b);
-}
-
-// Eq 29a-e (L393-403): Lambda(zeta) for direction x given P* = p_xx, sigma_bar, qtilde;
-// a P^1.1 e^{-P^2} and P^1.4 are evaluated through one log and exp (pow-free).
-struct WS14 { double pref, E, sC, cst; };
-__device__ __forceinline__ WS14 ws14_common(double Pdd, double sb, double qt2)
-{
-    WS14 w;
-    double lnP = log(Pdd);
-    double a = 1.4 * exp(1.1 * lnP - Pdd * Pdd);
-    double b = 0.9 * Pdd * exp(-0.5 * exp(1.4 * lnP));
-    double ss = sqrt(sb);
-    double C = sqrt((3.0 - 3.0 * sb) * Pdd);
-    w.E = 0.8 * C;
-    double B = 5.0 - 4.0 * ss + sqrt(fmax(10.0 - 16.0 * ss + 6.0 * sb, 0.0));
-    double Y = B + w.E * w.E - 2.0 * w.E * sqrt(B);
-    w.pref = (a * sb + b) / (2.0 * sb);
-    w.sC = 0.8 * sb * C;
-    w.cst = 4.0 * sb * sb * Y + 0.1 * qt2;
-    return w;
-}
-__device__ __forceinline__ double ws14_lambda(const WS14& w, double zeta)
-{
-    double rad = fmax(zeta * zeta - zeta * w.sC + w.cst, 0.0);      // floored (R6)
-    return w.pref * (zeta + sqrt(rad)) + w.E;
-}
-
-// lambda_min / lambda_max along x of an (index-swapped for y) state, Eqs 28-31 (L388-411).
-__device__ __forceinline__ void wavespeed14_x(const Params& p, const Star14& s, double sb,
-                                              double ux, double& lmin, double& lmax)
-{
-    double qt2 = s.hy * s.hy + s.hz * s.hz;
-    double qt = sqrt(qt2);                                           // Eq 28, qtilde >= 0 (R7)
-    double alpha = (0.6 * s.pxx - 0.38) * s.pxx + 0.35;              // Eq 29b
-    WS14 w = ws14_common(s.pxx, sb, qt2);
-    double kc = p.ws_scale * s.c;
-    lmax = ux + kc * ws14_lambda(w, s.hx + alpha * qt);
-    lmin = ux - kc * ws14_lambda(w, -s.hx + alpha * qt);             // Eq 30
-}
-// the same along y without swapping the state: P* = p_yy, q_d = h_y, qtilde from (h_x, h_z)
-__device__ __forceinline__ void wavespeed14_y(const Params& p, const Star14& s, double sb,
-                                              double uy, double& lmin, double& lmax)
-{
-    double qt2 = s.hx * s.hx + s.hz * s.hz;
-    double qt = sqrt(qt2);
-    double alpha = (0.6 * s.pyy - 0.38) * s.pyy + 0.35;
-    WS14 w = ws14_common(s.pyy, sb, qt2);
-    double kc = p.ws_scale * s.c;
-    lmax = uy + kc * ws14_lambda(w, s.hy + alpha * qt);
-    lmin = uy - kc * ws14_lambda(w, -s.hy + alpha * qt);
-}
-
-// Face evaluation along x: F = x-flux of Eq 16 (L169-181) with the closing moments Q_ijx,
-// R_ixjj, S_xiijj of Eqs 22-25 (L214-230) at sigma_bar; U = conserved moments of W; the
-// approximate wave speeds (Eqs 28-31).  Only what the x-flux needs is evaluated:
-//   B = 2 t2 p + 4 p^3 (Eq 25a), v = B^-1 h, a = p v,
-//   Q*_ijx = 2 [a_i (p^2)_jx + a_x (p^2)_ij + a_j (p^2)_ix]                       (Eqs 22, 25b)
-//   T_i = Q*_ixl w_l,  R*_ix = T_i/sb + 2(1-sb)(p^2)_ix + 3 p_ix                   (Eq 23)
-//   S*_x = (w.T)/sb^2 + 6 sqrt(sb) h_x + (1 - sqrt(sb)) (M v)_x                    (Eq 24)
-//   M = [2*27 p + 12 t3 p + 14 t2 p^2 + 60 p^3 + 20 p^4 - 6 t2 p - 54 p^2]         (Eq 25c, tr p = 3)
-// with p^3 = 3p^2 - I2 p + I3, p^4 = (9-I2)p^2 + (I3-3I2)p + 3I3 (Cayley-Hamilton, I1 = 3,
-// I2 = (9 - t2)/2, I3 = det p), so M = m2 p^2 + m1 p + m0.
-// The flux polynomials are written as F = u_x U + (pressure / heat-flux / closure terms).
-__device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[14],
-                                            double (&F)[14], double (&U)[14], double& lmin,
-                                            double& lmax)
-{
-    Star14 s;
-    nondim_sigma14(W, s);
-    const double sb = clamp_sigma(s.sigma, p.sigma_lim);
-    const double isb = 1.0 / sb, ss = sqrt(sb);
-
-    const double I2 = 0.5 * (9.0 - s.t2), I3 = s.I3;
-    const double t3 = 3.0 * s.t2 - 3.0 * I2 + 3.0 * I3;
-    // B = 12 p^2 + (2 t2 - 4 I2) p + 4 I3 I
-    const double bp = 2.0 * s.t2 - 4.0 * I2, b0 = 4.0 * I3;
-    const double Bxx = 12.0 * s.sxx + bp * s.pxx + b0, Bxy = 12.0 * s.sxy + bp * s.pxy;
-    const double Bxz = 12.0 * s.sxz + bp * s.pxz, Byy = 12.0 * s.syy + bp * s.pyy + b0;
-    const double Byz = 12.0 * s.syz + bp * s.pyz, Bzz = 12.0 * s.szz + bp * s.pzz + b0;
-    const double cxx = Byy * Bzz - Byz * Byz, cxy = Bxz * Byz - Bxy * Bzz;
-    const double cxz = Bxy * Byz - Bxz * Byy, cyy = Bxx * Bzz - Bxz * Bxz;
-    const double cyz = Bxy * Bxz - Bxx * Byz, czz = Bxx * Byy - Bxy * Bxy;
-    const double idB = 1.0 / (Bxx * cxx + Bxy * cxy + Bxz * cxz);
-    const double vx = (cxx * s.hx + cxy * s.hy + cxz * s.hz) * idB;
-    const double vy = (cxy * s.hx + cyy * s.hy + cyz * s.hz) * idB;
-    const double vz = (cxz * s.hx + cyz * s.hy + czz * s.hz) * idB;
-    const double ax = s.pxx * vx + s.pxy * vy + s.pxz * vz;
-    const double ay = s.pxy * vx + s.pyy * vy + s.pyz * vz;
-    const double az = s.pxz * vx + s.pyz * vy + s.pzz * vz;
-    // Q*_ijx
-    const double Qxx = 6.0 * ax * s.sxx;
-    const double Qxy = 2.0 * (2.0 * ax * s.sxy + ay * s.sxx);
-    const double Qxz = 2.0 * (2.0 * ax * s.sxz + az * s.sxx);
-    const double Qyy = 2.0 * (2.0 * ay * s.sxy + ax * s.syy);
-    const double Qyz = 2.0 * (ay * s.sxz + ax * s.syz + az * s.sxy);
-    const double Qzz = 2.0 * (2.0 * az * s.sxz + ax * s.szz);
-    // T_i = Q*_ixl w_l
-    const double Tx = Qxx * s.wx + Qxy * s.wy + Qxz * s.wz;
-    const double Ty = Qxy * s.wx + Qyy * s.wy + Qyz * s.wz;
-    const double Tz = Qxz * s.wx + Qyz * s.wy + Qzz * s.wz;
-    const double g = 2.0 * (1.0 - sb);
-    const double Rxs = Tx * isb + g * s.sxx + 3.0 * s.pxx;
-    const double Rys = Ty * isb + g * s.sxy + 3.0 * s.pxy;
-    const double Rzs = Tz * isb + g * s.sxz + 3.0 * s.pxz;
-    const double m2 = 14.0 * s.t2 + 306.0 - 20.0 * I2;
-    const double m1 = 54.0 - 6.0 * s.t2 + 12.0 * t3 - 120.0 * I2 + 20.0 * I3;
-    const double m0 = 120.0 * I3;
-    const double pax = s.pxx * ax + s.pxy * ay + s.pxz * az;          // (p^2 v)_x
-    const double Mvx = m2 * pax + m1 * ax + m0 * vx;
-    const double Sxs = (s.wx * Tx + s.wy * Ty + s.wz * Tz) * (isb * isb) + 6.0 * ss * s.hx
-                     + (1.0 - ss) * Mvx;
-    // re-dimensionalise: Q = rho c^3 Q*, R = rho c^4 R*, S = rho c^5 S*  (rho c^2 = P)
-    const double rc3 = s.Ph * s.c, rc4 = rc3 * s.c, rc5 = rc4 * s.c;
-    const double Qxxx = rc3 * Qxx, Qxyx = rc3 * Qxy, Qxzx = rc3 * Qxz;
-    const double Qyyx = rc3 * Qyy, Qyzx = rc3 * Qyz, Qzzx = rc3 * Qzz;
-    const double Rx = rc4 * Rxs, Ry = rc4 * Rys, Rz = rc4 * Rzs, Sx = rc5 * Sxs;
-
-    prim2cons14(W, U);
-    const double ux = W[1], uy = W[2], uz = W[3];
-    const double Pxx = W[4], Pxy = W[5], Pxz = W[6];
-    const double qx = W[10];
-    const double u2 = ux * ux + uy * uy + uz * uz;
-    const double uPx = ux * Pxx + uy * Pxy + uz * Pxz;                 // u_j P_jx
-    F[0] = U[1];                                                       // 16a
-    F[1] = ux * U[1] + Pxx;                                            // 16b
-    F[2] = ux * U[2] + Pxy;
-    F[3] = ux * U[3] + Pxz;
-    F[4] = ux * U[4] + 2.0 * ux * Pxx + Qxxx;                          // 16c
-    F[5] = ux * U[5] + ux * Pxy + uy * Pxx + Qxyx;
-    F[6] = ux * U[6] + ux * Pxz + uz * Pxx + Qxzx;
-    F[7] = ux * U[7] + 2.0 * uy * Pxy + Qyyx;
-    F[8] = ux * U[8] + uy * Pxz + uz * Pxy + Qyzx;
-    F[9] = ux * U[9] + 2.0 * uz * Pxz + Qzzx;
-    const double k1 = 2.0 * uPx + qx;                                  // 16d
-    F[10] = ux * U[10] + ux * k1 + u2 * Pxx + 2.0 * (ux * Qxxx + uy * Qxyx + uz * Qxzx) + Rx;
-    F[11] = ux * U[11] + uy * k1 + u2 * Pxy + 2.0 * (ux * Qxyx + uy * Qyyx + uz * Qyzx) + Ry;
-    F[12] = ux * U[12] + uz * k1 + u2 * Pxz + 2.0 * (ux * Qxzx + uy * Qyzx + uz * Qzzx) + Rz;
-    const double uuQ = ux * (ux * Qxxx + 2.0 * (uy * Qxyx + uz * Qxzx))
-                     + uy * (uy * Qyyx + 2.0 * uz * Qyzx) + uz * uz * Qzzx;
-    F[13] = ux * U[13] + 2.0 * u2 * k1 + 4.0 * (uuQ + ux * Rx + uy * Ry + uz * Rz) + Sx;   // 16e
-
-    wavespeed14_x(p, s, sb, ux, lmin, lmax);
-}
-
-// max(|lmin|,|lmax|) along x and y of a cell-centre state, for the CFL reduction (L434).
-// ok = false when rho <= 0 or P <= 0.
-__device__ __forceinline__ bool cell_speeds14(const Params& p, const double (&W)[14], double& sx,
-                                              double& sy)
-{
-    double Ph = W[4] + W[7] + W[9];
-    if (!(W[0] > 0.0) || !(Ph > 0.0)) { sx = sy = 0.0; return false; }
-    Star14 s;
-    nondim_sigma14(W, s);
-    const double sb = clamp_sigma(s.sigma, p.sigma_lim);
-    double a, b;
-    wavespeed14_x(p, s, sb, W[1], a, b);
-    sx = fmax(fabs(a), fabs(b));
-    wavespeed14_y(p, s, sb, W[2], a, b);
-    sy = fmax(fabs(a), fabs(b));
-    return true;
-}
 __device__ __forceinline__ bool cell_speed5(const Params& p, const double (&W)[5], double& sx)
 {
     if (!(W[0] > 0.0) || !(W[2] > 0.0)) { sx = 0.0; return false; }
@@ -440,33 +245,16 @@ __device__ __forceinline__ bool cell_speed5(const Params& p, const double (&W)[5
 __device__ __forceinline__ double inv_tau(const Params& p, double rho, double Ph)
 {
     if (p.tau_model == 1) return p.inv_tau_const;
-    if (p.tau_model == 2) return p.inv_tau_coef * rho * sqrt(8.0 * Ph / (3.14159265358979323846 * rho));
+    if (p.tau_model == 2) return p.inv_tau_coef * rho * fsqrt(8.0 * Ph * rcp(3.14159265358979323846 * rho));
     return 0.0;
 }
 
-// BGK source Eqs 17-18 (L185-194), times dt: Un += dt * C(W).
-__device__ __forceinline__ void add_source14(const double (&W)[14], double dt_over_tau,
-                                             double (&Un)[14])
-{
-    const double rho = W[0], ux = W[1], uy = W[2], uz = W[3];
-    const double Pxx = W[4], Pxy = W[5], Pxz = W[6], Pyy = W[7], Pyz = W[8], Pzz = W[9];
-    const double Ph = (Pxx + Pyy + Pzz) / 3.0;
-    const double k = -dt_over_tau;
-    Un[4] += k * (Pxx - Ph); Un[5] += k * Pxy; Un[6] += k * Pxz;
-    Un[7] += k * (Pyy - Ph); Un[8] += k * Pyz; Un[9] += k * (Pzz - Ph);
-    const double Pux = Pxx * ux + Pxy * uy + Pxz * uz;
-    const double Puy = Pxy * ux + Pyy * uy + Pyz * uz;
-    const double Puz = Pxz * ux + Pyz * uy + Pzz * uz;
-    Un[10] += k * (2.0 * Pux + W[10] - 2.0 * ux * Ph);
-    Un[11] += k * (2.0 * Puy + W[11] - 2.0 * uy * Ph);
-    Un[12] += k * (2.0 * Puz + W[12] - 2.0 * uz * Ph);
-    const double u2 = ux * ux + uy * uy + uz * uz;
-    const double uPu = ux * Pux + uy * Puy + uz * Puz;
-    const double uq = ux * W[10] + uy * W[11] + uz * W[12];
-    Un[13] += k * ((4.0 * uPu + 4.0 * uq + W[13]) - (4.0 * u2 * Ph + 15.0 * Ph * Ph / rho));
-}
-
 // HLL (L256-258; speeds combined as in DESIGN.md R12) or Rusanov (L258) interface flux.
+__device__ __forceinline__ double hll1(double SL, double SR, double SLR, double inv, double FL,
+                                       double FR, double UL, double UR)
+{
+    return (SR * FL - SL * FR + SLR * (UR - UL)) * inv;
+}
 template <int NM>
 __device__ __forceinline__ void numflux(int flux, const double (&FL)[NM], const double (&FR)[NM],
                                         const double (&UL)[NM], const double (&UR)[NM],
@@ -480,10 +268,333 @@ __device__ __forceinline__ void numflux(int flux, const double (&FL)[NM], const 
         return;
     }
     double SL = fmin(fmin(lminL, lminR), 0.0), SR = fmax(fmax(lmaxL, lmaxR), 0.0);
-    double inv = 1.0 / (SR - SL), SLR = SL * SR;
+    double inv = rcp(SR - SL), SLR = SL * SR;
 #pragma unroll
-    for (int m = 0; m < NM; ++m)
-        Fh[m] = (SR * FL[m] - SL * FR[m] + SLR * (UR[m] - UL[m])) * inv;
+    for (int m = 0; m < NM; ++m) Fh[m] = hll1(SL, SR, SLR, inv, FL[m], FR[m], UL[m], UR[m]);
+}
+
+// =========================================================================== 14-moment
+// Inverse of the conserved forms of Eq 16 (L169-181).  z-odd slots of U are not read and
+// z-odd slots of W are not written when Z = zero_t.
+template <class Z>
+__device__ __forceinline__ void cons2prim14(const double (&U)[14], double (&W)[14])
+{
+    const double rho = U[0], ir = rcp(rho);
+    const double ux = U[1] * ir, uy = U[2] * ir;
+    const Z uz = zget<Z>(U[3]) * ir;
+    const double Pxx = U[4] - rho * ux * ux, Pxy = U[5] - rho * ux * uy;
+    const Z Pxz = zget<Z>(U[6]) - rho * ux * uz;
+    const double Pyy = U[7] - rho * uy * uy;
+    const Z Pyz = zget<Z>(U[8]) - rho * uy * uz;
+    const double Pzz = U[9] - rho * uz * uz;
+    const double u2 = ux * ux + uy * uy + uz * uz, trP = Pxx + Pyy + Pzz;
+    const double Pux = Pxx * ux + Pxy * uy + Pxz * uz;
+    const double Puy = Pxy * ux + Pyy * uy + Pyz * uz;
+    const Z Puz = Pxz * ux + Pyz * uy + Pzz * uz;
+    const double e = rho * u2 + trP;
+    const double qx = U[10] - ux * e - 2.0 * Pux;
+    const double qy = U[11] - uy * e - 2.0 * Puy;
+    const Z qz = zget<Z>(U[12]) - uz * e - 2.0 * Puz;
+    const double uPu = ux * Pux + uy * Puy + uz * Puz, uq = ux * qx + uy * qy + uz * qz;
+    const double R = U[13] - rho * u2 * u2 - 2.0 * u2 * trP - 4.0 * uPu - 4.0 * uq;
+    W[0] = rho; W[1] = ux; W[2] = uy; zput(W[3], uz);
+    W[4] = Pxx; W[5] = Pxy; zput(W[6], Pxz); W[7] = Pyy; zput(W[8], Pyz); W[9] = Pzz;
+    W[10] = qx; W[11] = qy; zput(W[12], qz); W[13] = R;
+}
+
+template <class Z>
+__device__ __forceinline__ void prim2cons14(const double (&W)[14], double (&U)[14])
+{
+    const double rho = W[0], ux = W[1], uy = W[2];
+    const Z uz = zget<Z>(W[3]);
+    const double Pxx = W[4], Pxy = W[5], Pyy = W[7], Pzz = W[9];
+    const Z Pxz = zget<Z>(W[6]), Pyz = zget<Z>(W[8]), qz = zget<Z>(W[12]);
+    const double u2 = ux * ux + uy * uy + uz * uz, trP = Pxx + Pyy + Pzz;
+    const double Pux = Pxx * ux + Pxy * uy + Pxz * uz;
+    const double Puy = Pxy * ux + Pyy * uy + Pyz * uz;
+    const Z Puz = Pxz * ux + Pyz * uy + Pzz * uz;
+    const double e = rho * u2 + trP;
+    const double rux = rho * ux, ruy = rho * uy;
+    const Z ruz = rho * uz;
+    U[0] = rho; U[1] = rux; U[2] = ruy; zput(U[3], ruz);
+    U[4] = rux * ux + Pxx; U[5] = rux * uy + Pxy; zput(U[6], rux * uz + Pxz);
+    U[7] = ruy * uy + Pyy; zput(U[8], ruy * uz + Pyz); U[9] = ruz * uz + Pzz;
+    U[10] = ux * e + 2.0 * Pux + W[10];
+    U[11] = uy * e + 2.0 * Puy + W[11];
+    zput(U[12], uz * e + 2.0 * Puz + qz);
+    const double uPu = ux * Pux + uy * Puy + uz * Puz;
+    const double uq = ux * W[10] + uy * W[11] + uz * qz;
+    U[13] = rho * u2 * u2 + 2.0 * u2 * trP + 4.0 * uPu + 4.0 * uq + W[13];
+}
+
+// Dimensionless state (Eq 6 L75-81, rho* = 1): c = sqrt(P/rho), P = P_ii/3, p = P_ij/P (tr p = 3),
+// h = q/(rho c^3), Rs = R/(rho c^4); plus p^2, adj(p), det p, w = p^-1 h, and sigma (Eq 21 L210).
+template <class Z>
+struct Star14 {
+    double c, Ph;
+    double pxx, pxy, pyy, pzz;               // p
+    Z pxz, pyz;
+    double sxx, sxy, syy, szz;               // p^2
+    Z sxz, syz;
+    double t2, I3;                           // tr p^2, det p
+    double hx, hy, wx, wy;                   // h, w = p^-1 h
+    Z hz, wz;
+    double sigma;                            // Eq 21, unlimited
+};
+
+template <class Z>
+__device__ __forceinline__ void nondim_sigma14(const double (&W)[14], Star14<Z>& s)
+{
+    const double rho = W[0];
+    const double Ph = (W[4] + W[7] + W[9]) * (1.0 / 3.0);
+    const double iP = rcp(Ph), ir = rcp(rho);
+    const double c2 = Ph * ir, c = fsqrt(c2);
+    s.c = c; s.Ph = Ph;
+    s.pxx = W[4] * iP; s.pxy = W[5] * iP; s.pxz = zget<Z>(W[6]) * iP;
+    s.pyy = W[7] * iP; s.pyz = zget<Z>(W[8]) * iP; s.pzz = W[9] * iP;
+    const double ih = iP * (c * rho * iP);                 // 1/(rho c^3) = 1/(P c)
+    s.hx = W[10] * ih; s.hy = W[11] * ih; s.hz = zget<Z>(W[12]) * ih;
+    const double Rs = W[13] * rho * iP * iP;               // R/(rho c^4) = R rho / P^2
+    s.sxx = s.pxx * s.pxx + s.pxy * s.pxy + s.pxz * s.pxz;
+    s.sxy = s.pxx * s.pxy + s.pxy * s.pyy + s.pxz * s.pyz;
+    s.sxz = s.pxx * s.pxz + s.pxy * s.pyz + s.pxz * s.pzz;
+    s.syy = s.pxy * s.pxy + s.pyy * s.pyy + s.pyz * s.pyz;
+    s.syz = s.pxy * s.pxz + s.pyy * s.pyz + s.pyz * s.pzz;
+    s.szz = s.pxz * s.pxz + s.pyz * s.pyz + s.pzz * s.pzz;
+    s.t2 = s.sxx + s.syy + s.szz;
+    double X;
+    if constexpr (std::is_same<Z, zero_t>::value) {
+        // p = (2x2 block) (+) p_zz: w = block^-1 h, det p = p_zz det(block)
+        const double d2 = s.pxx * s.pyy - s.pxy * s.pxy;
+        const double id = rcp(d2);
+        s.I3 = s.pzz * d2;
+        s.wx = (s.pyy * s.hx - s.pxy * s.hy) * id;
+        s.wy = (s.pxx * s.hy - s.pxy * s.hx) * id;
+        X = s.hx * s.wx + s.hy * s.wy;
+    } else {
+        // adjugate (cofactors) of p and det p
+        const double axx = s.pyy * s.pzz - s.pyz * s.pyz, axy = s.pxz * s.pyz - s.pxy * s.pzz;
+        const double axz = s.pxy * s.pyz - s.pxz * s.pyy, ayy = s.pxx * s.pzz - s.pxz * s.pxz;
+        const double ayz = s.pxy * s.pxz - s.pxx * s.pyz, azz = s.pxx * s.pyy - s.pxy * s.pxy;
+        s.I3 = s.pxx * axx + s.pxy * axy + s.pxz * axz;
+        const double id = rcp(s.I3);
+        s.wx = (axx * s.hx + axy * s.hy + axz * s.hz) * id;
+        s.wy = (axy * s.hx + ayy * s.hy + ayz * s.hz) * id;
+        s.wz = (axz * s.hx + ayz * s.hy + azz * s.hz) * id;
+        X = s.hx * s.wx + s.hy * s.wy + s.hz * s.wz;
+    }
+    // Eq 21 with P_ii P_jj = 9: sigma = [b + sqrt(b^2 + 8 t2 X)]/(4 t2), b = 2 t2 + 9 - R*,
+    // X = h.p^-1.h; conjugate form when b < 0 (DESIGN.md R4)
+    const double b = 2.0 * s.t2 + 9.0 - Rs;
+    const double D = fsqrt(b * b + 8.0 * s.t2 * X);
+    const bool pos = b >= 0.0;
+    s.sigma = (pos ? b + D : 2.0 * X) * rcp(pos ? 4.0 * s.t2 : D - b);
+}
+
+// Quantities of Eq 29 that depend on sigma_bar only (shared by all directions of a state).
+struct SbTerms { double sb, ss, isb, B, sqB; };
+__device__ __forceinline__ SbTerms sb_terms(double sb)
+{
+    SbTerms t;
+    t.sb = sb; t.ss = fsqrt(sb); t.isb = rcp(sb);
+    t.B = 5.0 - 4.0 * t.ss + fsqrt(fmax(10.0 - 16.0 * t.ss + 6.0 * sb, 0.0));   // Eq 29e
+    t.sqB = fsqrt(t.B);
+    return t;
+}
+
+// Eq 29a-e (L393-403): lambda*_max and -lambda*_min along one direction given P* = p_dd, the
+// heat flux along (hd) and across (qt2 = sum of squares of the other two), sigma_bar terms.
+// a P^1.1 e^{-P^2} and P^1.4 go through one log and exp (pow-free); Y = B + E^2 - 2 E sqrt(B)
+// is evaluated as (sqrt(B) - E)^2; the radicand is floored at 0 (R6).
+__device__ __forceinline__ void ws14_dir(double Pdd, double hd, double qt2, const SbTerms& t,
+                                         double& lam_max, double& lam_min_neg)
+{
+    const double lnP = log(Pdd);
+    const double a = 1.4 * exp(1.1 * lnP - Pdd * Pdd);
+    const double b = 0.9 * Pdd * exp(-0.5 * exp(1.4 * lnP));
+    const double C = fsqrt((3.0 - 3.0 * t.sb) * Pdd);
+    const double E = 0.8 * C;
+    const double sY = t.sqB - E;
+    const double pref = (a * t.sb + b) * (0.5 * t.isb);
+    const double sC = 0.8 * t.sb * C;
+    const double cst = 4.0 * t.sb * t.sb * (sY * sY) + 0.1 * qt2;
+    const double qt = fsqrt(qt2);                                    // Eq 28, qtilde >= 0 (R7)
+    const double alpha = (0.6 * Pdd - 0.38) * Pdd + 0.35;            // Eq 29b
+    const double zp = hd + alpha * qt, zm = -hd + alpha * qt;        // Eq 30: q_d -> -q_d
+    const double rp = fmax(zp * zp - zp * sC + cst, 0.0), rm = fmax(zm * zm - zm * sC + cst, 0.0);
+    lam_max = pref * (zp + fsqrt(rp)) + E;
+    lam_min_neg = pref * (zm + fsqrt(rm)) + E;
+}
+
+// lambda_min / lambda_max along x of an (index-swapped for y) state, Eqs 28-31 (L388-411).
+template <class Z>
+__device__ __forceinline__ void wavespeed14_x(const Params& p, const Star14<Z>& s,
+                                              const SbTerms& t, double ux, double& lmin, double& lmax)
+{
+    double a, b;
+    ws14_dir(s.pxx, s.hx, s.hy * s.hy + s.hz * s.hz, t, a, b);
+    const double kc = p.ws_scale * s.c;
+    lmax = ux + kc * a; lmin = ux - kc * b;
+}
+// the same along y without swapping the state: P* = p_yy, q_d = h_y, qtilde from (h_x, h_z)
+template <class Z>
+__device__ __forceinline__ void wavespeed14_y(const Params& p, const Star14<Z>& s,
+                                              const SbTerms& t, double uy, double& lmin, double& lmax)
+{
+    double a, b;
+    ws14_dir(s.pyy, s.hy, s.hx * s.hx + s.hz * s.hz, t, a, b);
+    const double kc = p.ws_scale * s.c;
+    lmax = uy + kc * a; lmin = uy - kc * b;
+}
+
+// Face evaluation along x: F = x-flux of Eq 16 (L169-181) with the closing moments Q_ijx,
+// R_ixjj, S_xiijj of Eqs 22-25 (L214-230) at sigma_bar; U = conserved moments of W; the
+// approximate wave speeds (Eqs 28-31).  Only what the x-flux needs is evaluated:
+//   B = 2 t2 p + 4 p^3 (Eq 25a), v = B^-1 h, a = p v,
+//   Q*_ijx = 2 [a_i (p^2)_jx + a_x (p^2)_ij + a_j (p^2)_ix]                       (Eqs 22, 25b)
+//   T_i = Q*_ixl w_l,  R*_ix = T_i/sb + 2(1-sb)(p^2)_ix + 3 p_ix                   (Eq 23)
+//   S*_x = (w.T)/sb^2 + 6 sqrt(sb) h_x + (1 - sqrt(sb)) (M v)_x                    (Eq 24)
+//   M = [2*27 p + 12 t3 p + 14 t2 p^2 + 60 p^3 + 20 p^4 - 6 t2 p - 54 p^2]         (Eq 25c, tr p = 3)
+// with p^3 = 3p^2 - I2 p + I3, p^4 = (9-I2)p^2 + (I3-3I2)p + 3I3 (Cayley-Hamilton, I1 = 3,
+// I2 = (9 - t2)/2, I3 = det p), so M = m2 p^2 + m1 p + m0.
+// The flux polynomials are written as F = u_x U + (pressure / heat-flux / closure terms).
+// z-odd slots of F and U are left untouched when Z = zero_t.
+template <class Z>
+__device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[14],
+                                            double (&F)[14], double (&U)[14], double& lmin,
+                                            double& lmax)
+{
+    Star14<Z> s;
+    nondim_sigma14<Z>(W, s);
+    const SbTerms t = sb_terms(clamp_sigma(s.sigma, p.sigma_lim));
+    const double sb = t.sb, isb = t.isb, ss = t.ss;
+
+    const double I2 = 0.5 * (9.0 - s.t2), I3 = s.I3;
+    const double t3 = 3.0 * s.t2 - 3.0 * I2 + 3.0 * I3;
+    // B = 12 p^2 + (2 t2 - 4 I2) p + 4 I3 I
+    const double bp = 2.0 * s.t2 - 4.0 * I2, b0 = 4.0 * I3;
+    const double Bxx = 12.0 * s.sxx + bp * s.pxx + b0, Bxy = 12.0 * s.sxy + bp * s.pxy;
+    const double Byy = 12.0 * s.syy + bp * s.pyy + b0;
+    double vx, vy;
+    Z vz;
+    if constexpr (std::is_same<Z, zero_t>::value) {
+        const double idB = rcp(Bxx * Byy - Bxy * Bxy);           // 2x2 block; v_z = 0
+        vx = (Byy * s.hx - Bxy * s.hy) * idB;
+        vy = (Bxx * s.hy - Bxy * s.hx) * idB;
+    } else {
+        const double Bxz = 12.0 * s.sxz + bp * s.pxz, Byz = 12.0 * s.syz + bp * s.pyz;
+        const double Bzz = 12.0 * s.szz + bp * s.pzz + b0;
+        const double cxx = Byy * Bzz - Byz * Byz, cxy = Bxz * Byz - Bxy * Bzz;
+        const double cxz = Bxy * Byz - Bxz * Byy, cyy = Bxx * Bzz - Bxz * Bxz;
+        const double cyz = Bxy * Bxz - Bxx * Byz, czz = Bxx * Byy - Bxy * Bxy;
+        const double idB = rcp(Bxx * cxx + Bxy * cxy + Bxz * cxz);
+        vx = (cxx * s.hx + cxy * s.hy + cxz * s.hz) * idB;
+        vy = (cxy * s.hx + cyy * s.hy + cyz * s.hz) * idB;
+        vz = (cxz * s.hx + cyz * s.hy + czz * s.hz) * idB;
+    }
+    const double ax = s.pxx * vx + s.pxy * vy + s.pxz * vz;
+    const double ay = s.pxy * vx + s.pyy * vy + s.pyz * vz;
+    const Z az = s.pxz * vx + s.pyz * vy + s.pzz * vz;
+    // Q*_ijx
+    const double Qxx = 6.0 * ax * s.sxx;
+    const double Qxy = 2.0 * (2.0 * ax * s.sxy + ay * s.sxx);
+    const Z Qxz = 2.0 * (2.0 * ax * s.sxz + az * s.sxx);
+    const double Qyy = 2.0 * (2.0 * ay * s.sxy + ax * s.syy);
+    const Z Qyz = 2.0 * (ay * s.sxz + ax * s.syz + az * s.sxy);
+    const double Qzz = 2.0 * (2.0 * az * s.sxz + ax * s.szz);
+    // T_i = Q*_ixl w_l
+    const double Tx = Qxx * s.wx + Qxy * s.wy + Qxz * s.wz;
+    const double Ty = Qxy * s.wx + Qyy * s.wy + Qyz * s.wz;
+    const Z Tz = Qxz * s.wx + Qyz * s.wy + Qzz * s.wz;
+    const double g = 2.0 * (1.0 - sb);
+    const double Rxs = Tx * isb + g * s.sxx + 3.0 * s.pxx;
+    const double Rys = Ty * isb + g * s.sxy + 3.0 * s.pxy;
+    const Z Rzs = Tz * isb + g * s.sxz + 3.0 * s.pxz;
+    const double m2 = 14.0 * s.t2 + 306.0 - 20.0 * I2;
+    const double m1 = 54.0 - 6.0 * s.t2 + 12.0 * t3 - 120.0 * I2 + 20.0 * I3;
+    const double m0 = 120.0 * I3;
+    const double pax = s.pxx * ax + s.pxy * ay + s.pxz * az;          // (p^2 v)_x
+    const double Mvx = m2 * pax + m1 * ax + m0 * vx;
+    const double Sxs = (s.wx * Tx + s.wy * Ty + s.wz * Tz) * (isb * isb) + 6.0 * ss * s.hx
+                     + (1.0 - ss) * Mvx;
+    // re-dimensionalise: Q = rho c^3 Q*, R = rho c^4 R*, S = rho c^5 S*  (rho c^2 = P)
+    const double rc3 = s.Ph * s.c, rc4 = rc3 * s.c, rc5 = rc4 * s.c;
+    const double Qxxx = rc3 * Qxx, Qxyx = rc3 * Qxy, Qyyx = rc3 * Qyy, Qzzx = rc3 * Qzz;
+    const Z Qxzx = rc3 * Qxz, Qyzx = rc3 * Qyz;
+    const double Rx = rc4 * Rxs, Ry = rc4 * Rys, Sx = rc5 * Sxs;
+    const Z Rz = rc4 * Rzs;
+
+    prim2cons14<Z>(W, U);
+    const double ux = W[1], uy = W[2];
+    const Z uz = zget<Z>(W[3]);
+    const double Pxx = W[4], Pxy = W[5];
+    const Z Pxz = zget<Z>(W[6]);
+    const double qx = W[10];
+    const double u2 = ux * ux + uy * uy + uz * uz;
+    const double uPx = ux * Pxx + uy * Pxy + uz * Pxz;                 // u_j P_jx
+    F[0] = U[1];                                                       // 16a
+    F[1] = ux * U[1] + Pxx;                                            // 16b
+    F[2] = ux * U[2] + Pxy;
+    zput(F[3], ux * zget<Z>(U[3]) + Pxz);
+    F[4] = ux * U[4] + 2.0 * ux * Pxx + Qxxx;                          // 16c
+    F[5] = ux * U[5] + ux * Pxy + uy * Pxx + Qxyx;
+    zput(F[6], ux * zget<Z>(U[6]) + ux * Pxz + uz * Pxx + Qxzx);
+    F[7] = ux * U[7] + 2.0 * uy * Pxy + Qyyx;
+    zput(F[8], ux * zget<Z>(U[8]) + uy * Pxz + uz * Pxy + Qyzx);
+    F[9] = ux * U[9] + 2.0 * uz * Pxz + Qzzx;
+    const double k1 = 2.0 * uPx + qx;                                  // 16d
+    F[10] = ux * U[10] + ux * k1 + u2 * Pxx + 2.0 * (ux * Qxxx + uy * Qxyx + uz * Qxzx) + Rx;
+    F[11] = ux * U[11] + uy * k1 + u2 * Pxy + 2.0 * (ux * Qxyx + uy * Qyyx + uz * Qyzx) + Ry;
+    zput(F[12], ux * zget<Z>(U[12]) + uz * k1 + u2 * Pxz + 2.0 * (ux * Qxzx + uy * Qyzx + uz * Qzzx) + Rz);
+    const double uuQ = ux * (ux * Qxxx + 2.0 * (uy * Qxyx + uz * Qxzx))
+                     + uy * (uy * Qyyx + 2.0 * uz * Qyzx) + uz * uz * Qzzx;
+    F[13] = ux * U[13] + 2.0 * u2 * k1 + 4.0 * (uuQ + ux * Rx + uy * Ry + uz * Rz) + Sx;   // 16e
+
+    wavespeed14_x<Z>(p, s, t, ux, lmin, lmax);
+}
+
+// max(|lmin|,|lmax|) along x and y of a cell-centre state, for the CFL reduction (L434).
+// ok = false when rho <= 0 or P <= 0.
+template <class Z>
+__device__ __forceinline__ bool cell_speeds14(const Params& p, const double (&W)[14], double& sx,
+                                              double& sy)
+{
+    double Ph = W[4] + W[7] + W[9];
+    if (!(W[0] > 0.0) || !(Ph > 0.0)) { sx = sy = 0.0; return false; }
+    Star14<Z> s;
+    nondim_sigma14<Z>(W, s);
+    const SbTerms t = sb_terms(clamp_sigma(s.sigma, p.sigma_lim));
+    double a, b;
+    wavespeed14_x<Z>(p, s, t, W[1], a, b);
+    sx = fmax(fabs(a), fabs(b));
+    wavespeed14_y<Z>(p, s, t, W[2], a, b);
+    sy = fmax(fabs(a), fabs(b));
+    return true;
+}
+
+// BGK source Eqs 17-18 (L185-194), times dt: Un += dt * C(W).
+template <class Z>
+__device__ __forceinline__ void add_source14(const double (&W)[14], double dt_over_tau,
+                                             double (&Un)[14])
+{
+    const double rho = W[0], ux = W[1], uy = W[2];
+    const Z uz = zget<Z>(W[3]);
+    const double Pxx = W[4], Pxy = W[5], Pyy = W[7], Pzz = W[9];
+    const Z Pxz = zget<Z>(W[6]), Pyz = zget<Z>(W[8]), qz = zget<Z>(W[12]);
+    const double Ph = (Pxx + Pyy + Pzz) * (1.0 / 3.0);
+    const double k = -dt_over_tau;
+    Un[4] += k * (Pxx - Ph); Un[5] += k * Pxy; zadd(Un[6], k * Pxz);
+    Un[7] += k * (Pyy - Ph); zadd(Un[8], k * Pyz); Un[9] += k * (Pzz - Ph);
+    const double Pux = Pxx * ux + Pxy * uy + Pxz * uz;
+    const double Puy = Pxy * ux + Pyy * uy + Pyz * uz;
+    const Z Puz = Pxz * ux + Pyz * uy + Pzz * uz;
+    Un[10] += k * (2.0 * Pux + W[10] - 2.0 * ux * Ph);
+    Un[11] += k * (2.0 * Puy + W[11] - 2.0 * uy * Ph);
+    zadd(Un[12], k * (2.0 * Puz + qz - 2.0 * uz * Ph));
+    const double u2 = ux * ux + uy * uy + uz * uz;
+    const double uPu = ux * Pux + uy * Puy + uz * Puz;
+    const double uq = ux * W[10] + uy * W[11] + uz * qz;
+    Un[13] += k * ((4.0 * uPu + 4.0 * uq + W[13]) - (4.0 * u2 * Ph + 15.0 * Ph * Ph * rcp(rho)));
 }
 
 }  // namespace mm

@@ -1,31 +1,55 @@
 // mm_strip14.cuh -- the fused 14-moment 2-D time step (steps a2-a9 of DESIGN.md section 2).
 //
-// One WARP owns a strip of 31 cells in x and marches through a chunk of rows in y; warps never
-// synchronise with one another.  Lane l owns the x-interface between strip cells l-1 and l
-// (32 interfaces for 31 cells) and the y-interfaces and the update of strip cell l (l < 31).
-// Per warp, in shared memory:
-//   ring  [4][14][35]  primitives of the rows r-2 .. r+1 (cells x0-2 .. x0+32), a ring over r;
-//   cons  [2][14][35]  conserved rows in flight: filled by cp.async one row ahead of use, so the
-//                      HBM latency of row r+2 hides behind the x pass of row r at no register cost;
-//   acc   [14][32]     per-lane partial update of the row being assembled.
-// Row iteration r:  G_r (y-interface r-1|r) -> finish row r-1 in the scheme's order of operations (x then y then source),
-// (acc - dt/dy (G_r - G_{r-1})) + dt C(W_{r-1}) (a8), store, cell-centre wave speeds of the new
-// state -> running CFL maximum (a9); then row r: x-interfaces, neighbour flux by warp shuffle,
-// acc = U_r - dt/dx (F_{i+1} - F_i).  The two interface directions run through
-// ONE copy of the slope / closure / wave-speed / HLL code (a non-unrolled loop over the
-// direction), which keeps the kernel inside the instruction cache.
+// One WARP owns a strip of 30 cells in x and marches through a chunk of rows in y; warps never
+// synchronise with one another.  Per warp, in shared memory (NV = moments carried: 14, or the
+// 10 z-even ones on the z-symmetric path):
+//   ring  [4][NV][34]  primitives of the rows r-2 .. r+1 (cells x0-2 .. x0+31), a ring over r;
+//   cons  [2][NV][34]  conserved rows in flight: filled by cp.async one row ahead of use, so the
+//                      HBM latency of row r+2 hides behind the work on row r at no register cost;
+//   acc   [NV][32]     partial update of the row being assembled;
+//   hsv   [NV][32]     half slopes in y of the previous row (each slope is computed once).
+// Every interface is evaluated in one form: the lane holds a centre cell C with its two
+// neighbours M and P along the direction, computes C's limited half slope h (a3), obtains the
+// half slope hM of M from the lane / row that computed it, and evaluates the interface M|C
+// from the face states W_M + hM and W_C - h (a4-a7).
+//   y (d = 0): lane l, C = cell l of row r, M = row r-1; hM from `hsv`; G_r completes row r-1:
+//              U^{n+1} = acc - dt/dy G_r + dt C(W) (a8), store, wave speeds of the new state
+//              into the running CFL maximum (a9); then acc = U_r + dt/dy G_r.  The product
+//              dt/dy G_r is rounded on its own both times (no FMA contraction), so that equal
+//              fluxes through the two y faces of a cell cancel exactly.
+//   x (d = 1): lane L, C = cell L-1 of row r, M = cell L-2; hM by shuffle from lane L-1;
+//              acc(cell L-1) -= dt/dx (F from lane L+1 - own F).
+// The two directions run through ONE copy of the slope / closure / wave-speed / HLL code (a
+// non-unrolled loop over d), which keeps the kernel inside the instruction cache.
 #pragma once
 #include "mm_kernels.cuh"
 
 namespace mm {
 
-constexpr int kSW = 31;                 // cells per strip
-constexpr int kRW = 35;                 // staged cells per row: 2 + 31 + 2
-constexpr int kRingD = 4 * 14 * kRW;    // doubles
-constexpr int kConsD = 2 * 14 * kRW;
-constexpr int kAccD = 14 * 32;
-constexpr int kWarpSmemD = kRingD + kConsD + kAccD;
-constexpr int kStripWPB = 2;            // warps per block (a container only)
+constexpr int kSW = 30;                 // cells per strip
+constexpr int kRW = 34;                 // staged cells per row: 2 + 30 + 2
+#ifndef MM_STRIP_WPB
+#define MM_STRIP_WPB 2
+#endif
+constexpr int kStripWPB = MM_STRIP_WPB; // warps per block (a container only)
+
+// Moments carried by a kernel variant and their compact numbering.
+template <bool ZS>
+struct Mom {
+    static constexpr int NV = ZS ? 10 : 14;
+    __host__ __device__ static constexpr int full(int k)          // compact -> moment index
+    {
+        const int t[14] = {0, 1, 2, 4, 5, 7, 9, 10, 11, 13, 0, 0, 0, 0};
+        return ZS ? t[k] : k;
+    }
+    __host__ __device__ static constexpr int compact(int m)       // moment index -> compact
+    {
+        const int t[14] = {0, 1, 2, -1, 3, 4, -1, 5, -1, 6, 7, 8, -1, 9};
+        return ZS ? t[m] : m;
+    }
+    __host__ __device__ static constexpr int cswap(int k) { return compact(swap_xy(full(k))); }
+    static constexpr int warp_smem_doubles = 4 * NV * kRW + 2 * NV * kRW + 2 * NV * 32;
+};
 
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
 {
@@ -35,55 +59,15 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// Interface flux from the four stencil cells (am | a || b | bp) along one direction.  q0..q3
-// point at moment plane 0 of those cells, ps is the plane stride.  MUSCL on primitives
-// (L262-264), both face states through the closure (eval_face14), HLL / Rusanov.  For the y
-// direction (swap) the state is index-swapped on load (L414); the caller swaps the flux back.
-__device__ __forceinline__ void iface_flux14(const Params& p, const double* __restrict__ q0,
-                                             const double* __restrict__ q1,
-                                             const double* __restrict__ q2,
-                                             const double* __restrict__ q3, int ps, bool swap,
-                                             double (&Fh)[14])
-{
-    constexpr int NM = 14;
-    double WL[NM], WR[NM];
-    if (p.limiter != 0 && p.shared_limiter) {
-        double Wam[NM], Wa[NM], Wb[NM], Wbp[NM], ha[NM], hb[NM];
-#pragma unroll
-        for (int k = 0; k < NM; ++k) {
-            const int o = (swap ? swap_xy(k) : k) * ps;
-            Wam[k] = q0[o]; Wa[k] = q1[o]; Wb[k] = q2[o]; Wbp[k] = q3[o];
-        }
-        half_slopes<NM>(p, Wam, Wa, Wb, ha);
-        half_slopes<NM>(p, Wa, Wb, Wbp, hb);
-#pragma unroll
-        for (int k = 0; k < NM; ++k) { WL[k] = Wa[k] + ha[k]; WR[k] = Wb[k] - hb[k]; }
-    } else {
-#pragma unroll
-        for (int k = 0; k < NM; ++k) {
-            const int o = (swap ? swap_xy(k) : k) * ps;
-            const double am = q0[o], a = q1[o], b = q2[o], bp = q3[o];
-            double ha = 0.0, hb = 0.0;
-            if (p.limiter != 0) {
-                const double d = b - a;
-                ha = 0.5 * limited_slope(p.limiter, a - am, d);
-                hb = 0.5 * limited_slope(p.limiter, d, bp - b);
-            }
-            WL[k] = a + ha; WR[k] = b - hb;
-        }
-    }
-    double FL[NM], UL[NM], FR[NM], UR[NM], lminL, lmaxL, lminR, lmaxR;
-    eval_face14(p, WL, FL, UL, lminL, lmaxL);
-    eval_face14(p, WR, FR, UR, lminR, lmaxR);
-    numflux<NM>(p.flux, FL, FR, UL, UR, lminL, lmaxL, lminR, lmaxR, Fh);
-}
-
 // Work decomposition: item = (strip, chunk); chunk c covers rows [c ny / nchunks, (c+1) ny / nchunks).
-__global__ void __launch_bounds__(32 * kStripWPB, 8 / kStripWPB)
+template <bool ZS, int MINB>
+__global__ void __launch_bounds__(32 * kStripWPB, MINB)
 k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl,
                int slot_next, int nstrips, int nchunks)
 {
-    constexpr int NM = 14, RS = NM * kRW;           // doubles per staged row
+    using Z = typename std::conditional<ZS, zero_t, double>::type;
+    using M = Mom<ZS>;
+    constexpr int NM = 14, NV = M::NV, RS = NV * kRW;          // RS: doubles per staged row
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int item = blockIdx.x * kStripWPB + warp;
@@ -93,13 +77,16 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
     const int y0 = (int)((long long)chunk * p.ny / nchunks);
     const int y1 = (int)((long long)(chunk + 1) * p.ny / nchunks);
     if (y1 <= y0) return;
-    double* ring = smem + warp * kWarpSmemD;
-    double* cons = ring + kRingD;
-    double* acc = cons + kConsD;
+    double* ring = smem + warp * M::warp_smem_doubles;
+    double* cons = ring + 4 * RS;
+    double* acc = cons + 2 * RS;
+    double* hsv = acc + NV * 32;
     const size_t plane = (size_t)p.rows * p.pitch;
-    const bool cell_ok = lane < kSW && x0 + lane < p.nx;
-    const bool xif_ok = x0 + lane <= p.nx;
-    const size_t ccol = (size_t)x0 + lane + 2;       // padded column of the lane's cell
+    const int ncell = min(kSW, p.nx - x0);            // cells of this strip
+    const int ncol = min(kRW, p.nx + 4 - x0);         // staged columns that exist
+    const bool cell_ok = lane < ncell;                // y phase: the lane's cell is cell `lane`
+    const bool xcell_ok = lane >= 1 && lane - 1 < ncell;  // x phase: cell lane-1 is updated
+    const size_t ccol = (size_t)x0 + lane + 2;        // padded column of the lane's cell (y phase)
 
     if (ctrl->skip) {                  // failed / past t_end: carry the state over unchanged
         if (cell_ok)
@@ -111,18 +98,17 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
     }
     const double dt = ctrl->dt;
     const double dtdx = dt / p.dx, dtdy = dt / p.dy;
-    const int ncol = min(kRW, p.nx + 4 - x0);        // staged columns that exist
 
     auto load_row = [&](int r, int cslot) {          // interior row r in [-2, ny+1] -> cons[cslot]
         const double* src = Uin + (size_t)(r + 2) * p.pitch + x0;
         double* dst = cons + cslot * RS;
         if (lane < ncol) {
 #pragma unroll
-            for (int m = 0; m < NM; ++m) cp_async8(dst + m * kRW + lane, src + m * plane + lane);
+            for (int k = 0; k < NV; ++k) cp_async8(dst + k * kRW + lane, src + M::full(k) * plane + lane);
         }
         if (lane + 32 < ncol) {
 #pragma unroll
-            for (int m = 0; m < NM; ++m) cp_async8(dst + m * kRW + 32 + lane, src + m * plane + 32 + lane);
+            for (int k = 0; k < NV; ++k) cp_async8(dst + k * kRW + 32 + lane, src + M::full(k) * plane + 32 + lane);
         }
         cp_async_commit();
     };
@@ -133,10 +119,10 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
         for (int c = lane; c < ncol; c += 32) {
             double U[NM], W[NM];
 #pragma unroll
-            for (int m = 0; m < NM; ++m) U[m] = src[m * kRW + c];
-            cons2prim14(U, W);
+            for (int k = 0; k < NV; ++k) U[M::full(k)] = src[k * kRW + c];
+            cons2prim14<Z>(U, W);
 #pragma unroll
-            for (int m = 0; m < NM; ++m) dst[m * kRW + c] = W[m];
+            for (int k = 0; k < NV; ++k) dst[k * kRW + c] = W[M::full(k)];
         }
     };
 
@@ -151,74 +137,132 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
 
     double rate = 0.0, speed = 0.0;
     int bad = 0;
-    double Gp[NM];                                   // y-interface flux of the previous row
-#pragma unroll
-    for (int m = 0; m < NM; ++m) Gp[m] = 0.0;
-    for (int r = y0; r <= y1; ++r) {
+    for (int r = y0 - 1; r <= y1; ++r) {
         const int cs = (r - y0) & 1;
 #pragma unroll 1
         for (int d = 0; d < 2; ++d) {
-            const double *q0, *q1, *q2, *q3;
+            const double *qm, *qc, *qp;              // plane 0 of the cells M, C, P
             bool act;
-            if (d == 0) {                            // y-interface between rows r-1 and r
+            if (d == 0) {                            // y: C = (row r, cell lane)
                 const double* b = ring + lane + 2;
-                q0 = b + (r & 3) * RS; q1 = b + ((r + 1) & 3) * RS;
-                q2 = b + ((r + 2) & 3) * RS; q3 = b + ((r + 3) & 3) * RS;
+                qm = b + ((r + 1) & 3) * RS; qc = b + ((r + 2) & 3) * RS; qp = b + ((r + 3) & 3) * RS;
                 act = cell_ok;
-            } else {                                 // x-interface between cells lane-1 and lane of row r
-                if (r == y1) break;
+            } else {                                 // x: C = (row r, cell lane-1)
+                if (r < y0 || r == y1) break;
                 __syncwarp();                        // every lane has taken U_r out of cons[cs]
                 load_row(r + 2, cs);
-                const double* b = ring + ((r + 2) & 3) * RS + lane;
-                q0 = b; q1 = b + 1; q2 = b + 2; q3 = b + 3;
-                act = xif_ok;
+                qm = ring + ((r + 2) & 3) * RS + lane; qc = qm + 1; qp = qm + 2;
+                act = lane + 2 < ncol;
             }
-            double Fh[NM];
+            // ---- a3: limited half slope of C; face states of the interface M|C
+            double WL[NM], WR[NM];
+            {
+                double Wm[NV], Wc[NV], Wp[NV], h[NV];
+                if (act) {
 #pragma unroll
-            for (int m = 0; m < NM; ++m) Fh[m] = 0.0;
-            if (act) iface_flux14(p, q0, q1, q2, q3, kRW, d == 0, Fh);
+                    for (int k = 0; k < NV; ++k) {
+                        const int o = (d == 0 ? M::cswap(k) : k) * kRW;
+                        Wm[k] = qm[o]; Wc[k] = qc[o]; Wp[k] = qp[o];
+                    }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) { Wm[k] = 1.0; Wc[k] = 1.0; Wp[k] = 1.0; }
+                }
+                if (p.limiter == 0) {
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) h[k] = 0.0;
+                } else if (p.shared_limiter) {
+                    PsiMin pm;
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) pm.add(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
+                    const double q = 0.25 * pm.psi();
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) h[k] = q * ((Wc[k] - Wm[k]) + (Wp[k] - Wc[k]));
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NV; ++k)
+                        h[k] = 0.5 * limited_slope(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
+                }
+                if (d == 0) {
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) {
+                        const double hm = hsv[k * 32 + lane];
+                        hsv[k * 32 + lane] = h[k];
+                        WL[M::full(k)] = Wm[k] + hm; WR[M::full(k)] = Wc[k] - h[k];
+                    }
+                    if (r < y0) continue;            // first pass of a chunk: slope of row y0-1 only
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) {
+                        const double hm = __shfl_up_sync(0xffffffffu, h[k], 1);
+                        WL[M::full(k)] = Wm[k] + hm; WR[M::full(k)] = Wc[k] - h[k];
+                    }
+                }
+            }
+            // ---- a4-a7: both face states through the closure, HLL / Rusanov
+            double Fh[NV];
+            {
+                double FL[NM], UL[NM], FR[NM], UR[NM], lminL, lmaxL, lminR, lmaxR;
+                eval_face14<Z>(p, WL, FL, UL, lminL, lmaxL);
+                eval_face14<Z>(p, WR, FR, UR, lminR, lmaxR);
+                if (p.flux == 1) {
+                    const double S = fmax(fmax(fabs(lminL), fabs(lmaxL)), fmax(fabs(lminR), fabs(lmaxR)));
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) {
+                        const int m = M::full(k);
+                        Fh[k] = 0.5 * (FL[m] + FR[m]) - 0.5 * S * (UR[m] - UL[m]);
+                    }
+                } else {
+                    const double SL = fmin(fmin(lminL, lminR), 0.0), SR = fmax(fmax(lmaxL, lmaxR), 0.0);
+                    const double inv = rcp(SR - SL), SLR = SL * SR;
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) {
+                        const int m = M::full(k);
+                        Fh[k] = hll1(SL, SR, SLR, inv, FL[m], FR[m], UL[m], UR[m]);
+                    }
+                }
+            }
             if (d == 0) {
                 if (cell_ok) {
-                    double G[NM];
+                    double G[NV];                    // back to unswapped numbering (L414)
 #pragma unroll
-                    for (int m = 0; m < NM; ++m) G[m] = Fh[swap_xy(m)];
+                    for (int k = 0; k < NV; ++k) G[k] = Fh[M::cswap(k)];
                     if (r > y0) {                    // row r-1 is complete (a8), then a9 on the new state
                         double Un[NM], W[NM];
                         const double* w = ring + ((r + 1) & 3) * RS + lane + 2;
 #pragma unroll
-                        for (int m = 0; m < NM; ++m) {
-                            Un[m] = acc[m * 32 + lane] - dtdy * (G[m] - Gp[m]);
-                            W[m] = w[m * kRW];
+                        for (int k = 0; k < NV; ++k) {
+                            Un[M::full(k)] = __dsub_rn(acc[k * 32 + lane], __dmul_rn(dtdy, G[k]));
+                            W[M::full(k)] = w[k * kRW];
                         }
                         if (p.tau_model != 0)
-                            add_source14(W, dt * inv_tau(p, W[0], (W[4] + W[7] + W[9]) / 3.0), Un);
+                            add_source14<Z>(W, dt * inv_tau(p, W[0], (W[4] + W[7] + W[9]) * (1.0 / 3.0)), Un);
+                        double* out = Uout + (size_t)(r + 1) * p.pitch + ccol;
 #pragma unroll
-                        for (int m = 0; m < NM; ++m)
-                            Uout[m * plane + (size_t)(r + 1) * p.pitch + ccol] = Un[m];
+                        for (int m = 0; m < NM; ++m) {
+                            if (ZS && z_odd(m)) out[m * plane] = 0.0;
+                            else out[m * plane] = Un[m];
+                        }
                         double rr, ss;
-                        cell_rate<NM>(p, Un, rr, ss, bad);
+                        cell_rate<NM, Z>(p, Un, rr, ss, bad);
                         rate = fmax(rate, rr); speed = fmax(speed, ss);
                     }
-#pragma unroll
-                    for (int m = 0; m < NM; ++m) Gp[m] = G[m];
                     if (r < y1) {
 #pragma unroll
-                        for (int m = 0; m < NM; ++m)
-                            acc[m * 32 + lane] = cons[cs * RS + m * kRW + lane + 2];
+                        for (int k = 0; k < NV; ++k)
+                            acc[k * 32 + lane] = __dadd_rn(cons[cs * RS + k * kRW + lane + 2], __dmul_rn(dtdy, G[k]));
                     }
                 }
             } else {
-                double Fn[NM];
+                __syncwarp();                        // acc of row r was written by the y phase
 #pragma unroll
-                for (int m = 0; m < NM; ++m) Fn[m] = __shfl_down_sync(0xffffffffu, Fh[m], 1);
-                if (cell_ok) {
-#pragma unroll
-                    for (int m = 0; m < NM; ++m)
-                        acc[m * 32 + lane] = acc[m * 32 + lane] - dtdx * (Fn[m] - Fh[m]);
+                for (int k = 0; k < NV; ++k) {
+                    const double Fn = __shfl_down_sync(0xffffffffu, Fh[k], 1);
+                    if (xcell_ok) acc[k * 32 + lane - 1] = acc[k * 32 + lane - 1] - dtdx * (Fn - Fh[k]);
                 }
             }
         }
-        if (r < y1) {                                // row r+2 has landed: primitives into the slot of row r-2
+        if (r >= y0 && r < y1) {                     // row r+2 has landed: primitives into the slot of row r-2
             cp_async_wait_all(); __syncwarp();
             convert_row(r + 2, cs);
             __syncwarp();

@@ -2,7 +2,7 @@
 // update (the "algorithmic flops" of the roofline line).
 // mm_physics.cuh is compiled on the HOST with `double` replaced by a counting type; the
 // composition below mirrors what the fused step kernel does for ONE cell with no tile overhead:
-//   1 cons->prim, 2 interfaces (x and y: slopes of both cells, 2 face evaluations, HLL),
+//   1 cons->prim, per direction 1 limited slope and 1 interface (2 face evaluations, HLL),
 //   the update, the BGK source and the tail CFL evaluation of the new state.
 // Convention: each + - * / sqrt exp log = 1 (an FMA is 2); comparisons, fabs, fmin/fmax,
 // negation and copies = 0.  Measurement tooling only; nothing here is linked into libmm.so.
@@ -39,6 +39,7 @@ inline cnt fmax(cnt a, cnt b) { return cnt(std::fmax(a.v, b.v)); }
 inline cnt fmin(cnt a, double b) { return cnt(std::fmin(a.v, b)); }
 inline cnt fmax(cnt a, double b) { return cnt(std::fmax(a.v, b)); }
 
+#include <type_traits>
 #define MM_OPCOUNT_HOST
 #define __device__
 #define __host__
@@ -47,23 +48,52 @@ inline cnt fmax(cnt a, double b) { return cnt(std::fmax(a.v, b)); }
 #include "mm_physics.cuh"
 using namespace mm;
 
+// one limited half slope of cell c from its neighbours (computed once per cell and direction)
 template <int NM>
-static void interface(const Params& p, const cnt (&Wam)[NM], const cnt (&Wa)[NM], const cnt (&Wb)[NM],
-                      const cnt (&Wbp)[NM], cnt (&Fh)[NM])
+static void half_slope(const Params& p, const cnt (&Wm)[NM], const cnt (&Wc)[NM], const cnt (&Wp)[NM],
+                       cnt (&h)[NM], bool zs)
 {
-    cnt ha[NM], hb[NM], WL[NM], WR[NM];
-    half_slopes<NM>(p, Wam, Wa, Wb, ha);
-    half_slopes<NM>(p, Wa, Wb, Wbp, hb);
-    for (int k = 0; k < NM; ++k) { WL[k] = Wa[k] + ha[k]; WR[k] = Wb[k] - hb[k]; }
-    cnt FL[NM], UL[NM], FR[NM], UR[NM], a, b, c, d;
-    if constexpr (NM == 5) { eval_face5(p, WL, FL, UL, a, b); eval_face5(p, WR, FR, UR, c, d); }
-    else { eval_face14(p, WL, FL, UL, a, b); eval_face14(p, WR, FR, UR, c, d); }
-    numflux<NM>(p.flux, FL, FR, UL, UR, a, b, c, d, Fh);
+    PsiMin pm;
+    for (int k = 0; k < NM; ++k) {
+        if (NM == 14 && zs && z_odd(k)) continue;
+        if (p.shared_limiter) pm.add(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
+        else h[k] = 0.5 * limited_slope(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
+    }
+    if (p.shared_limiter) {
+        const cnt q = 0.25 * pm.psi();
+        for (int k = 0; k < NM; ++k) {
+            if (NM == 14 && zs && z_odd(k)) continue;
+            h[k] = q * ((Wc[k] - Wm[k]) + (Wp[k] - Wc[k]));
+        }
+    }
 }
 
-template <int NM>
+// interface M|C: face states from the two half slopes, two face evaluations, HLL
+template <int NM, class Z>
+static void interface(const Params& p, const cnt (&Wm)[NM], const cnt (&hm)[NM], const cnt (&Wc)[NM],
+                      const cnt (&hc)[NM], cnt (&Fh)[NM])
+{
+    constexpr bool zs = std::is_same<Z, zero_t>::value;
+    cnt WL[NM], WR[NM];
+    for (int k = 0; k < NM; ++k) {
+        if (NM == 14 && zs && z_odd(k)) continue;
+        WL[k] = Wm[k] + hm[k]; WR[k] = Wc[k] - hc[k];
+    }
+    cnt FL[NM], UL[NM], FR[NM], UR[NM], a, b, c, d;
+    if constexpr (NM == 5) { eval_face5(p, WL, FL, UL, a, b); eval_face5(p, WR, FR, UR, c, d); }
+    else { eval_face14<Z>(p, WL, FL, UL, a, b); eval_face14<Z>(p, WR, FR, UR, c, d); }
+    const cnt SL = fmin(fmin(a, c), 0.0), SR = fmax(fmax(b, d), 0.0);
+    const cnt inv = rcp(SR - SL), SLR = SL * SR;
+    for (int k = 0; k < NM; ++k) {
+        if (NM == 14 && zs && z_odd(k)) continue;
+        Fh[k] = hll1(SL, SR, SLR, inv, FL[k], FR[k], UL[k], UR[k]);
+    }
+}
+
+template <int NM, class Z>
 static long long one_cell(Params p, int ndim)
 {
+    constexpr bool zs = std::is_same<Z, zero_t>::value;
     // four smooth, non-equilibrium neighbouring states (all limiter branches active)
     cnt W[4][NM];
     for (int c = 0; c < 4; ++c) {
@@ -74,25 +104,30 @@ static long long one_cell(Params p, int ndim)
         } else {
             const cnt w[14] = {1.0 + e, 0.3 + e, -0.2 + e, 0.1 + e, 1.1 + e, 0.05 + e, 0.02 + e, 0.9 + e,
                                0.03 + e, 1.0 + e, 0.2 + e, -0.1 + e, 0.05 + e, 16.0 + 9.0 * e};
-            for (int k = 0; k < 14; ++k) W[c][k] = w[k];
+            for (int k = 0; k < 14; ++k) W[c][k] = (zs && z_odd(k)) ? cnt(0.0) : w[k];
         }
     }
-    cnt U[NM], Wc[NM], Fw[NM], Fe[NM], Un[NM];
-    if constexpr (NM == 5) prim2cons5(W[1], U); else prim2cons14(W[1], U);
+    cnt U[NM], Wc[NM], Fw[NM], Fe[NM], Un[NM], hm[NM], hc[NM];
+    if constexpr (NM == 5) prim2cons5(W[1], U); else prim2cons14<Z>(W[1], U);
+    half_slope<NM>(p, W[0], W[1], W[2], hm, zs);       // the neighbour's slope (its own cost)
     cnt::ops = 0;
-    if constexpr (NM == 5) cons2prim5(U, Wc); else cons2prim14(U, Wc);
+    if constexpr (NM == 5) cons2prim5(U, Wc); else cons2prim14<Z>(U, Wc);
     const cnt dt = 1e-3, dtdx = dt / p.dx, dtdy = dt / p.dy;
-    for (int d = 0; d < ndim; ++d) {          // each cell owns one interface per direction
-        interface<NM>(p, W[0], W[1], W[2], W[3], Fe);
-        for (int k = 0; k < NM; ++k) Fw[k] = Fe[k] * 0.99;   // neighbour's flux (not counted twice)
-        cnt::ops -= NM;
-        for (int k = 0; k < NM; ++k) Un[k] = (d == 0 ? U[k] : Un[k]) - (d == 0 ? dtdx : dtdy) * (Fe[k] - Fw[k]);
+    for (int d = 0; d < ndim; ++d) {          // each cell owns one slope and one interface per direction
+        half_slope<NM>(p, W[1], W[2], W[3], hc, zs);
+        interface<NM, Z>(p, W[1], hm, W[2], hc, Fe);
+        for (int k = 0; k < NM; ++k) Fw[k] = Fe[k];         // neighbour's flux (not counted twice)
+        for (int k = 0; k < NM; ++k) {
+            if (NM == 14 && zs && z_odd(k)) continue;
+            // x: acc = U - dtdx (F' - F); y: acc + dtdy G, then - dtdy G'  (2 flops each per moment)
+            Un[k] = (d == 0 ? U[k] : Un[k]) - (d == 0 ? dtdx : dtdy) * (Fe[k] - Fw[k]);
+        }
     }
     if constexpr (NM == 5) add_source5(Wc, dt * inv_tau(p, Wc[0], Wc[2]), Un);
-    else add_source14(Wc, dt * inv_tau(p, Wc[0], (Wc[4] + Wc[7] + Wc[9]) / 3.0), Un);
+    else add_source14<Z>(Wc, dt * inv_tau(p, Wc[0], (Wc[4] + Wc[7] + Wc[9]) * (1.0 / 3.0)), Un);
     cnt Wn[NM], sx, sy;
     if constexpr (NM == 5) { cons2prim5(Un, Wn); cell_speed5(p, Wn, sx); sx = sx / p.dx; }
-    else { cons2prim14(Un, Wn); cell_speeds14(p, Wn, sx, sy); sx = fmax(sx / p.dx, sy / p.dy); }
+    else { cons2prim14<Z>(Un, Wn); cell_speeds14<Z>(p, Wn, sx, sy); sx = fmax(sx / p.dx, sy / p.dy); }
     return cnt::ops;
 }
 
@@ -103,10 +138,10 @@ int main()
     p.inv_tau_coef = 100.0; p.tau_model = 2; p.limiter = 1; p.flux = 0;
     for (int shared = 0; shared < 2; ++shared) {
         p.shared_limiter = shared;
-        printf("kernel_flops_per_cell_update_14_%s %lld\n", shared ? "shared_limiter" : "per_variable_limiter",
-               one_cell<14>(p, 2));
-        printf("kernel_flops_per_cell_update_5_%s %lld\n", shared ? "shared_limiter" : "per_variable_limiter",
-               one_cell<5>(p, 1));
+        const char* nm = shared ? "shared_limiter" : "per_variable_limiter";
+        printf("kernel_flops_per_cell_update_14_%s %lld\n", nm, one_cell<14, double>(p, 2));
+        printf("kernel_flops_per_cell_update_14_zsym_%s %lld\n", nm, one_cell<14, zero_t>(p, 2));
+        printf("kernel_flops_per_cell_update_5_%s %lld\n", nm, one_cell<5, double>(p, 1));
     }
     return 0;
 }

@@ -24,7 +24,8 @@ MAX_BANDS = 8
 EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim", "mm_step",
            "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
            "mm_cfl_dt", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
-           "mm_measure_fp64_peak", "mm_destroy", "mm_strerror"]
+           "mm_measure_fp64_peak", "mm_selftest_fastmath", "mm_set_fast_path", "mm_fast_path_active",
+           "mm_destroy", "mm_strerror"]
 
 _dp = C.POINTER(C.c_double)
 
@@ -84,6 +85,9 @@ def lib() -> C.CDLL:
     L.mm_profile_end.restype = i
     L.mm_profile_end.argtypes = [vp, _dp, C.POINTER(C.c_longlong)]
     L.mm_measure_fp64_peak.restype, L.mm_measure_fp64_peak.argtypes = i, [vp, i, _dp]
+    L.mm_selftest_fastmath.restype, L.mm_selftest_fastmath.argtypes = i, [vp, i, _dp, _dp]
+    L.mm_set_fast_path.restype, L.mm_set_fast_path.argtypes = i, [vp, i]
+    L.mm_fast_path_active.restype, L.mm_fast_path_active.argtypes = i, [vp]
     L.mm_destroy.restype, L.mm_destroy.argtypes = None, [vp]
     L.mm_strerror.restype, L.mm_strerror.argtypes = C.c_char_p, [i]
     _lib = L
@@ -114,6 +118,15 @@ def mm_measure_fp64_peak(repeats: int = 5, stream=None) -> float:
     tf = C.c_double()
     _check(lib().mm_measure_fp64_peak(C.c_void_p(st.cuda_stream), repeats, C.byref(tf)))
     return tf.value
+
+
+def mm_selftest_fastmath(n: int = 1 << 22, stream=None):
+    """Max error (units of 2^-53 relative) of the library's reciprocal and square root vs IEEE."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    a, b = C.c_double(), C.c_double()
+    _check(lib().mm_selftest_fastmath(C.c_void_p(st.cuda_stream), n, C.byref(a), C.byref(b)))
+    return a.value, b.value
 
 
 class Solver:
@@ -247,6 +260,14 @@ class Solver:
         ms, n = C.c_double(), C.c_longlong()
         _check(self._L.mm_profile_end(self._h, C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def set_fast_path(self, allow: bool):
+        """Allow (default) or forbid the z-symmetric kernel variant (include/mm.h)."""
+        _check(self._L.mm_set_fast_path(self._h, 1 if allow else 0))
+
+    @property
+    def fast_path_active(self) -> bool:
+        return bool(self._L.mm_fast_path_active(self._h))
 
     @property
     def launches(self) -> int:
