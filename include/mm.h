@@ -137,10 +137,11 @@ int mm_profile_end(mm_solver *s, double *step_kernel_ms, long long *launches);
  * `stream` (cudaStream_t): 2 flop per FMA, best of `repeats` launches.  This is the roofline
  * denominator of this FP64-ALU-bound method; MEASURED_PEAKS.json has no FP64 entry. */
 int mm_measure_fp64_peak(void *stream, int repeats, double *tflops);
-/* Accuracy of the library's branch-free reciprocal and square root (Newton on the hardware
- * seeds) against IEEE division / sqrt over n pseudo-random normal arguments spanning
- * 1e-30 .. 1e30 on `stream`: max relative error of each, in units of 2^-53. */
-int mm_selftest_fastmath(void *stream, int n, double *max_ulp_rcp, double *max_ulp_sqrt);
+/* Accuracy of the library's branch-free elementary functions against the IEEE / libm ones over
+ * n pseudo-random arguments on `stream`: max relative error, in units of 2^-53, of
+ * max_ulp[0] reciprocal and [1] square root (arguments spanning 1e-30 .. 1e30),
+ * [2] exp on (-30, 0], [3] P^1.1 and P^1.4 on (0, 4)  (the functions of Eq 29c-d). */
+int mm_selftest_fastmath(void *stream, int n, double max_ulp[4]);
 
 void mm_destroy(mm_solver *s);
 const char *mm_strerror(int status);

@@ -480,20 +480,20 @@ int mm_measure_fp64_peak(void* stream, int repeats, double* tflops)
     return MM_OK;
 }
 
-int mm_selftest_fastmath(void* stream, int n, double* max_ulp_rcp, double* max_ulp_sqrt)
+int mm_selftest_fastmath(void* stream, int n, double* max_ulp)
 {
-    if (n < 1 || !max_ulp_rcp || !max_ulp_sqrt) return MM_EINVAL;
+    if (n < 1 || !max_ulp) return MM_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     unsigned long long* d = nullptr;
-    MM_CUDA(cudaMalloc(&d, 2 * sizeof(unsigned long long)));   // measurement scratch only
-    cudaMemsetAsync(d, 0, 2 * sizeof(unsigned long long), st);
-    k_fastmath_test<<<296, 256, 0, st>>>(n, d, d + 1);
-    unsigned long long h[2] = {0, 0};
+    MM_CUDA(cudaMalloc(&d, 4 * sizeof(unsigned long long)));   // measurement scratch only
+    cudaMemsetAsync(d, 0, 4 * sizeof(unsigned long long), st);
+    k_fastmath_test<<<296, 256, 0, st>>>(n, d, d + 1, d + 2, d + 3);
+    unsigned long long h[4] = {0, 0, 0, 0};
     cudaError_t e = cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     cudaFree(d);
     if (e != cudaSuccess) return cuda_fail(e, "k_fastmath_test");
-    *max_ulp_rcp = bits2d(h[0]); *max_ulp_sqrt = bits2d(h[1]);
+    for (int k = 0; k < 4; ++k) max_ulp[k] = bits2d(h[k]);
     return MM_OK;
 }
 

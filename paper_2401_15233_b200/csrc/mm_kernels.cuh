@@ -383,9 +383,10 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, doubl
 
 
 // max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x)
-__global__ void k_fastmath_test(int n, unsigned long long* err_rcp_bits, unsigned long long* err_sqrt_bits)
+__global__ void k_fastmath_test(int n, unsigned long long* err_rcp_bits, unsigned long long* err_sqrt_bits,
+                                unsigned long long* err_exp_bits, unsigned long long* err_pow_bits)
 {
-    double er = 0.0, es = 0.0;
+    double er = 0.0, es = 0.0, ee = 0.0, ep = 0.0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         unsigned long long z = (unsigned long long)i * 0x9E3779B97F4A7C15ull + 0x2401152330ull;
         z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
@@ -394,10 +395,19 @@ __global__ void k_fastmath_test(int n, unsigned long long* err_rcp_bits, unsigne
         const double r0 = 1.0 / x, s0 = sqrt(x);
         er = fmax(er, fabs(rcp(x) - r0) / r0);
         es = fmax(es, fabs(fsqrt(x) - s0) / s0);
+        const double xe = -30.0 * (m - 1.0), e0 = exp(xe);              // (-30, 0]
+        ee = fmax(ee, fabs(exp_neg(xe) - e0) / e0);
+        const double P = 4.0 * (m - 1.0) + 1e-6 * (double)(z & 1023);   // (0, 4)
+        double p11, p14;
+        pow_11_14(P, p11, p14);
+        const double r11 = pow(P, 1.1), r14 = pow(P, 1.4);
+        if (P > 0.0) ep = fmax(ep, fmax(fabs(p11 - r11) / r11, fabs(p14 - r14) / r14));
     }
     const double ulp = 1.1102230246251565e-16;
     atomic_max_pos(err_rcp_bits, er / ulp);
     atomic_max_pos(err_sqrt_bits, es / ulp);
+    atomic_max_pos(err_exp_bits, ee / ulp);
+    atomic_max_pos(err_pow_bits, ep / ulp);
 }
 
 }  // namespace mm

@@ -52,9 +52,13 @@ __host__ __device__ __forceinline__ void zadd(double&, zero_t) {}
 #ifdef MM_OPCOUNT_HOST
 __forceinline__ double rcp(double x) { return 1.0 / x; }
 __forceinline__ double fsqrt(double x) { return sqrt(x); }
+__forceinline__ double exp_neg(double x) { return exp(x); }
+__forceinline__ void pow_11_14(double P, double& p11, double& p14) { p11 = pow(P, 1.1); p14 = pow(P, 1.4); }
 #elif defined(MM_EXACT_MATH)
 __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
 __device__ __forceinline__ double fsqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ double exp_neg(double x) { return exp(x); }
+__device__ __forceinline__ void pow_11_14(double P, double& p11, double& p14) { p11 = pow(P, 1.1); p14 = pow(P, 1.4); }
 #else
 __device__ __forceinline__ double rcp(double x)
 {
@@ -70,15 +74,57 @@ __device__ __forceinline__ double fsqrt(double x)
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double s0 = x * y;
-    const double e = fma(-s0, y, 1.0);         // 1 - x y^2
+    const double e = fma(-s0, y, 1.0);         // 1 - x y^2, |e| <~ 2^-19
     const double pe = fma(0.375, e, 0.5);
-    const double y1 = fma(y * e, pe, y);       // y (1 + e/2 + 3e^2/8): error ~ e^3
-    double s = x * y1;
-    const double r = fma(-s, s, x);            // final Newton correction of the root itself
-    s = fma(r, 0.5 * y1, s);
+    const double s = fma(s0 * e, pe, s0);      // x y (1 + e/2 + 3e^2/8): error ~ e^3
     // the hardware seed flushes subnormal arguments to zero (-> inf): everything below 1e-290
     // is returned as 0 (absolute error < 1e-145); negative or NaN arguments still give NaN
     return fabs(x) < 1e-290 ? 0.0 : s;
+}
+// exp(x) for x <= 0 (the arguments of Eq 29c-d are -P*^2 and -P*^1.4/2): no overflow handling,
+// x below -700 is clamped (result < 1e-304).  n = rint(x log2 e), r = x - n ln2 (two-term),
+// degree-13 Taylor polynomial on |r| <= 0.347 (truncation 4e-18), scaled by 2^n.
+__device__ __forceinline__ double exp_neg(double x)
+{
+    x = fmax(x, -700.0) + (x - x);                                   // keeps NaN
+    const double t = fma(x, 1.4426950408889634, 6755399441055744.0);  // 1.5 * 2^52: n in the low word
+    const double n = t - 6755399441055744.0;
+    double r = fma(n, -6.93147180369123816490e-01, x);
+    r = fma(n, -1.90821492927058770002e-10, r);
+    double q = 1.6059043836821613e-10;                                // 1/13!
+    q = fma(q, r, 2.08767569878681e-09);                              // 1/12!
+    q = fma(q, r, 2.505210838544172e-08);
+    q = fma(q, r, 2.755731922398589e-07);
+    q = fma(q, r, 2.7557319223985893e-06);
+    q = fma(q, r, 2.48015873015873e-05);
+    q = fma(q, r, 1.984126984126984e-04);
+    q = fma(q, r, 1.388888888888889e-03);
+    q = fma(q, r, 8.333333333333333e-03);
+    q = fma(q, r, 4.1666666666666664e-02);
+    q = fma(q, r, 1.6666666666666666e-01);
+    q = fma(q, r, 0.5);
+    q = fma(q, r, 1.0);
+    q = fma(q, r, 1.0);
+    const int k = __double2loint(t);
+    return q * __hiloint2double((k + 1023) << 20, 0);
+}
+// P^1.1 and P^1.4 (Eq 29c-d) for P > 0 without log / pow: z ~ P^-0.1 from the fp32 units,
+// two Newton steps z <- z (1 + (1 - P z^10)/10) (error 5.5 e^2 per step), u = P z^9 ~ P^0.1
+// with one quasi-Newton step on u^10 = P, then P^1.1 = P u, P^1.4 = P u^4.  P <= 0 gives NaN.
+__device__ __forceinline__ void pow_11_14(double P, double& p11, double& p14)
+{
+    double z = (double)__powf((float)P, -0.1f);
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const double z2 = z * z, z4 = z2 * z2, z5 = z4 * z, z10 = z5 * z5;
+        z = fma(0.1 * z, fma(-P, z10, 1.0), z);
+    }
+    const double z2 = z * z, z4 = z2 * z2, z9 = z4 * z4 * z;
+    double u = P * z9;
+    const double u2 = u * u, u4 = u2 * u2, u5 = u4 * u;
+    u = fma(-0.1 * z9, fma(u5, u5, -P), u);
+    const double v2 = u * u;
+    p11 = P * u; p14 = P * (v2 * v2);
 }
 #endif
 
@@ -404,14 +450,15 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
 
 // Eq 29a-e (L393-403): lambda*_max and -lambda*_min along one direction given P* = p_dd, the
 // heat flux along (hd) and across (qt2 = sum of squares of the other two), sigma_bar terms.
-// a P^1.1 e^{-P^2} and P^1.4 go through one log and exp (pow-free); Y = B + E^2 - 2 E sqrt(B)
+// P^1.1 and P^1.4 come from pow_11_14 (no log / pow), the exponentials from exp_neg; Y = B + E^2 - 2 E sqrt(B)
 // is evaluated as (sqrt(B) - E)^2; the radicand is floored at 0 (R6).
 __device__ __forceinline__ void ws14_dir(double Pdd, double hd, double qt2, const SbTerms& t,
                                          double& lam_max, double& lam_min_neg)
 {
-    const double lnP = log(Pdd);
-    const double a = 1.4 * exp(1.1 * lnP - Pdd * Pdd);
-    const double b = 0.9 * Pdd * exp(-0.5 * exp(1.4 * lnP));
+    double p11, p14;
+    pow_11_14(Pdd, p11, p14);
+    const double a = 1.4 * p11 * exp_neg(-(Pdd * Pdd));
+    const double b = 0.9 * Pdd * exp_neg(-0.5 * p14);
     const double C = fsqrt((3.0 - 3.0 * t.sb) * Pdd);
     const double E = 0.8 * C;
     const double sY = t.sqB - E;

@@ -3,7 +3,7 @@
 // One WARP owns a strip of 30 cells in x and marches through a chunk of rows in y; warps never
 // synchronise with one another.  Per warp, in shared memory (NV = moments carried: 14, or the
 // 10 z-even ones on the z-symmetric path):
-//   ring  [4][NV][34]  primitives of the rows r-2 .. r+1 (cells x0-2 .. x0+31), a ring over r;
+//   ring  [3][NV][34]  primitives of the rows r-1 .. r+1 (cells x0-2 .. x0+31), a ring over r;
 //   cons  [2][NV][34]  conserved rows in flight: filled by cp.async one row ahead of use, so the
 //                      HBM latency of row r+2 hides behind the work on row r at no register cost;
 //   acc   [NV][32]     partial update of the row being assembled;
@@ -48,7 +48,7 @@ struct Mom {
         return ZS ? t[m] : m;
     }
     __host__ __device__ static constexpr int cswap(int k) { return compact(swap_xy(full(k))); }
-    static constexpr int warp_smem_doubles = 4 * NV * kRW + 2 * NV * kRW + 2 * NV * 32;
+    static constexpr int warp_smem_doubles = 3 * NV * kRW + 2 * NV * kRW + 2 * NV * 32;
 };
 
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
@@ -78,7 +78,7 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
     const int y1 = (int)((long long)(chunk + 1) * p.ny / nchunks);
     if (y1 <= y0) return;
     double* ring = smem + warp * M::warp_smem_doubles;
-    double* cons = ring + 4 * RS;
+    double* cons = ring + 3 * RS;
     double* acc = cons + 2 * RS;
     double* hsv = acc + NV * 32;
     const size_t plane = (size_t)p.rows * p.pitch;
@@ -112,9 +112,9 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
         }
         cp_async_commit();
     };
-    auto convert_row = [&](int r, int cslot) {       // cons[cslot] -> primitives in the ring (a2)
+    auto convert_row = [&](int cslot, int rslot) {   // cons[cslot] -> primitives in ring[rslot] (a2)
         const double* src = cons + cslot * RS;
-        double* dst = ring + ((r + 2) & 3) * RS;
+        double* dst = ring + rslot * RS;
 #pragma unroll 1
         for (int c = lane; c < ncol; c += 32) {
             double U[NM], W[NM];
@@ -128,12 +128,13 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
 
     load_row(y0 - 2, 0); load_row(y0 - 1, 1);
     cp_async_wait_all(); __syncwarp();
-    convert_row(y0 - 2, 0); convert_row(y0 - 1, 1);
+    convert_row(0, 0); convert_row(1, 1);
     __syncwarp();
-    load_row(y0, 0); load_row(y0 + 1, 1);
+    load_row(y0, 0); load_row(y0 + 1, 1);            // stay in cons: U of rows y0, y0+1
     cp_async_wait_all(); __syncwarp();
-    convert_row(y0, 0); convert_row(y0 + 1, 1);
+    convert_row(0, 2);
     __syncwarp();
+    int sm = 0, sc = 1, sp = 2;                      // ring slots of the rows r-1, r, r+1
 
     double rate = 0.0, speed = 0.0;
     int bad = 0;
@@ -145,13 +146,13 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
             bool act;
             if (d == 0) {                            // y: C = (row r, cell lane)
                 const double* b = ring + lane + 2;
-                qm = b + ((r + 1) & 3) * RS; qc = b + ((r + 2) & 3) * RS; qp = b + ((r + 3) & 3) * RS;
+                qm = b + sm * RS; qc = b + sc * RS; qp = b + sp * RS;
                 act = cell_ok;
             } else {                                 // x: C = (row r, cell lane-1)
                 if (r < y0 || r == y1) break;
                 __syncwarp();                        // every lane has taken U_r out of cons[cs]
                 load_row(r + 2, cs);
-                qm = ring + ((r + 2) & 3) * RS + lane; qc = qm + 1; qp = qm + 2;
+                qm = ring + sc * RS + lane; qc = qm + 1; qp = qm + 2;
                 act = lane + 2 < ncol;
             }
             // ---- a3: limited half slope of C; face states of the interface M|C
@@ -229,7 +230,7 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
                     for (int k = 0; k < NV; ++k) G[k] = Fh[M::cswap(k)];
                     if (r > y0) {                    // row r-1 is complete (a8), then a9 on the new state
                         double Un[NM], W[NM];
-                        const double* w = ring + ((r + 1) & 3) * RS + lane + 2;
+                        const double* w = ring + sm * RS + lane + 2;
 #pragma unroll
                         for (int k = 0; k < NV; ++k) {
                             Un[M::full(k)] = __dsub_rn(acc[k * 32 + lane], __dmul_rn(dtdy, G[k]));
@@ -262,10 +263,11 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
                 }
             }
         }
-        if (r >= y0 && r < y1) {                     // row r+2 has landed: primitives into the slot of row r-2
+        if (r < y1) {                                // row r+2 has landed: primitives into the slot of row r-1
             cp_async_wait_all(); __syncwarp();
-            convert_row(r + 2, cs);
+            convert_row(cs, sm);
             __syncwarp();
+            const int t = sm; sm = sc; sc = sp; sp = t;
         }
     }
 #pragma unroll

@@ -4,7 +4,7 @@
 // composition below mirrors what the fused step kernel does for ONE cell with no tile overhead:
 //   1 cons->prim, per direction 1 limited slope and 1 interface (2 face evaluations, HLL),
 //   the update, the BGK source and the tail CFL evaluation of the new state.
-// Convention: each + - * / sqrt exp log = 1 (an FMA is 2); comparisons, fabs, fmin/fmax,
+// Convention: each + - * / sqrt exp pow = 1 (an FMA is 2); comparisons, fabs, fmin/fmax,
 // negation and copies = 0.  Measurement tooling only; nothing here is linked into libmm.so.
 #include <cmath>
 #include <cstdio>
@@ -33,6 +33,7 @@ R(<) R(>) R(<=) R(>=) R(==)
 inline cnt sqrt(cnt a) { ++cnt::ops; return cnt(std::sqrt(a.v)); }
 inline cnt exp(cnt a) { ++cnt::ops; return cnt(std::exp(a.v)); }
 inline cnt log(cnt a) { ++cnt::ops; return cnt(std::log(a.v)); }
+inline cnt pow(cnt a, double b) { ++cnt::ops; return cnt(std::pow(a.v, b)); }
 inline cnt fabs(cnt a) { return cnt(std::fabs(a.v)); }
 inline cnt fmin(cnt a, cnt b) { return cnt(std::fmin(a.v, b.v)); }
 inline cnt fmax(cnt a, cnt b) { return cnt(std::fmax(a.v, b.v)); }

@@ -196,10 +196,11 @@ def test_fast_path_selection(mm):
 
 
 def test_fastmath_accuracy(mm):
-    """The branch-free reciprocal / square root of the CUDA path are within 2 units of 2^-53
-    of IEEE division / sqrt over 4 M arguments spanning 1e-30 .. 1e30."""
-    e_rcp, e_sqrt = mm.mm_selftest_fastmath(1 << 22)
-    assert 0.0 <= e_rcp <= 2.0 and 0.0 <= e_sqrt <= 2.0, (e_rcp, e_sqrt)
+    """The branch-free reciprocal, square root, exp and P^1.1 / P^1.4 of the CUDA path against
+    IEEE division / sqrt and libm over 4 M arguments, in units of 2^-53 relative."""
+    e_rcp, e_sqrt, e_exp, e_pow = mm.mm_selftest_fastmath(1 << 22)
+    assert 0.0 < e_rcp <= 2.0 and 0.0 <= e_sqrt <= 2.0, (e_rcp, e_sqrt)
+    assert 0.0 < e_exp <= 4.0 and 0.0 < e_pow <= 16.0, (e_exp, e_pow)
 
 
 def test_smooth14_transmissive(mm, mmo):
