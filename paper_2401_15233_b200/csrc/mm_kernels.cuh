@@ -382,11 +382,63 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, doubl
 }
 
 
-// max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x)
-__global__ void k_fastmath_test(int n, unsigned long long* err_rcp_bits, unsigned long long* err_sqrt_bits,
-                                unsigned long long* err_exp_bits, unsigned long long* err_pow_bits)
+// cos(pi n / d) for integers n >= 0, d > 0, reduced exactly to the first quadrant so that the
+// argument handed to cospi is at most 1/2 and carries one rounding only
+__device__ inline double cos_quarter(int n, int d)
 {
-    double er = 0.0, es = 0.0, ee = 0.0, ep = 0.0;
+    n %= 2 * d;                                   // period 2 pi
+    if (n > d) n = 2 * d - n;                     // cos(2 pi - x) = cos x
+    const bool neg = 2 * n > d;                   // cos(pi - x) = -cos x
+    if (neg) n = d - n;
+    const double c = cospi((double)n / (double)d);
+    return neg ? -c : c;
+}
+
+// Builds the AbTable (mm_physics.cuh): one thread per (interval, function).  Chebyshev
+// interpolation of the direct formula at 14 nodes, then re-expansion in powers of the local
+// coordinate t in [-1, 1] (coefficients stored highest power first, for Horner).
+__global__ void k_ab_table(double* __restrict__ tab)
+{
+    constexpr int N = AbTable::kDeg + 1;
+    const int i = blockIdx.x, f = threadIdx.x;              // interval, 0 = a / 1 = b
+    if (i >= AbTable::kIntervals || f >= 2) return;
+    const double half = 1.0 / AbTable::inv_half(i), mid = AbTable::lower(i) + half;
+    double fv[N], c[N];
+    for (int j = 0; j < N; ++j) {
+        const double P = mid + half * cos_quarter(2 * j + 1, 2 * N);
+        double a, b;
+        ab_direct(P, &a, &b);
+        fv[j] = f == 0 ? a : b;
+    }
+    for (int k = 0; k < N; ++k) {                           // Chebyshev coefficients, compensated sums
+        double hi = 0.0, lo = 0.0;
+        for (int j = 0; j < N; ++j) {
+            const double w = cos_quarter(k * (2 * j + 1), 2 * N);
+            const double pr = fv[j] * w, pe = fma(fv[j], w, -pr);          // two-product
+            const double sm = hi + pr, bb = sm - hi;                       // two-sum
+            lo += (hi - (sm - bb)) + (pr - bb) + pe;
+            hi = sm;
+        }
+        c[k] = (hi + lo) * (k == 0 ? 1.0 : 2.0) / N;
+    }
+    double m[N], Tkm1[N], Tk[N];                            // monomial coefficients of sum c_k T_k
+    for (int j = 0; j < N; ++j) { m[j] = 0.0; Tkm1[j] = 0.0; Tk[j] = 0.0; }
+    Tkm1[0] = 1.0; Tk[1] = 1.0;                             // T_0, T_1
+    m[0] += c[0]; m[1] += c[1];
+    for (int k = 2; k < N; ++k) {
+        double Tn[N];
+        for (int j = 0; j < N; ++j) Tn[j] = (j > 0 ? 2.0 * Tk[j - 1] : 0.0) - Tkm1[j];
+        for (int j = 0; j < N; ++j) { m[j] = fma(c[k], Tn[j], m[j]); Tkm1[j] = Tk[j]; Tk[j] = Tn[j]; }
+    }
+    double* out = tab + i * AbTable::kStride;
+    for (int j = 0; j < N; ++j) out[f * N + j] = m[N - 1 - j];
+}
+
+// max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x), and of the
+// tabulated a(P*), b(P*) against the direct formulas on (0, 3]
+__global__ void k_fastmath_test(int n, unsigned long long* err_bits, const double* __restrict__ tab)
+{
+    double er = 0.0, es = 0.0, eab = 0.0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         unsigned long long z = (unsigned long long)i * 0x9E3779B97F4A7C15ull + 0x2401152330ull;
         z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
@@ -395,19 +447,18 @@ __global__ void k_fastmath_test(int n, unsigned long long* err_rcp_bits, unsigne
         const double r0 = 1.0 / x, s0 = sqrt(x);
         er = fmax(er, fabs(rcp(x) - r0) / r0);
         es = fmax(es, fabs(fsqrt(x) - s0) / s0);
-        const double xe = -30.0 * (m - 1.0), e0 = exp(xe);              // (-30, 0]
-        ee = fmax(ee, fabs(exp_neg(xe) - e0) / e0);
-        const double P = 4.0 * (m - 1.0) + 1e-6 * (double)(z & 1023);   // (0, 4)
-        double p11, p14;
-        pow_11_14(P, p11, p14);
-        const double r11 = pow(P, 1.1), r14 = pow(P, 1.4);
-        if (P > 0.0) ep = fmax(ep, fmax(fabs(p11 - r11) / r11, fabs(p14 - r14) / r14));
+        const double P = 3.0 * (m - 1.0) + 1e-7 * (double)(z & 1023);   // (0, 3]: realizable p_dd
+        if (P > 0.0) {
+            double a0, b0, a1, b1;
+            ab_direct(P, &a0, &b0);
+            ab_eval(tab, P, a1, b1);
+            eab = fmax(eab, fmax(fabs(a1 - a0) / a0, fabs(b1 - b0) / b0));
+        }
     }
     const double ulp = 1.1102230246251565e-16;
-    atomic_max_pos(err_rcp_bits, er / ulp);
-    atomic_max_pos(err_sqrt_bits, es / ulp);
-    atomic_max_pos(err_exp_bits, ee / ulp);
-    atomic_max_pos(err_pow_bits, ep / ulp);
+    atomic_max_pos(err_bits, er / ulp);
+    atomic_max_pos(err_bits + 1, es / ulp);
+    atomic_max_pos(err_bits + 2, eab / ulp);
 }
 
 }  // namespace mm

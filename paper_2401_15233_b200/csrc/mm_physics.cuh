@@ -52,13 +52,9 @@ __host__ __device__ __forceinline__ void zadd(double&, zero_t) {}
 #ifdef MM_OPCOUNT_HOST
 __forceinline__ double rcp(double x) { return 1.0 / x; }
 __forceinline__ double fsqrt(double x) { return sqrt(x); }
-__forceinline__ double exp_neg(double x) { return exp(x); }
-__forceinline__ void pow_11_14(double P, double& p11, double& p14) { p11 = pow(P, 1.1); p14 = pow(P, 1.4); }
 #elif defined(MM_EXACT_MATH)
 __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
 __device__ __forceinline__ double fsqrt(double x) { return sqrt(x); }
-__device__ __forceinline__ double exp_neg(double x) { return exp(x); }
-__device__ __forceinline__ void pow_11_14(double P, double& p11, double& p14) { p11 = pow(P, 1.1); p14 = pow(P, 1.4); }
 #else
 __device__ __forceinline__ double rcp(double x)
 {
@@ -81,51 +77,6 @@ __device__ __forceinline__ double fsqrt(double x)
     // is returned as 0 (absolute error < 1e-145); negative or NaN arguments still give NaN
     return fabs(x) < 1e-290 ? 0.0 : s;
 }
-// exp(x) for x <= 0 (the arguments of Eq 29c-d are -P*^2 and -P*^1.4/2): no overflow handling,
-// x below -700 is clamped (result < 1e-304).  n = rint(x log2 e), r = x - n ln2 (two-term),
-// degree-13 Taylor polynomial on |r| <= 0.347 (truncation 4e-18), scaled by 2^n.
-__device__ __forceinline__ double exp_neg(double x)
-{
-    x = fmax(x, -700.0) + (x - x);                                   // keeps NaN
-    const double t = fma(x, 1.4426950408889634, 6755399441055744.0);  // 1.5 * 2^52: n in the low word
-    const double n = t - 6755399441055744.0;
-    double r = fma(n, -6.93147180369123816490e-01, x);
-    r = fma(n, -1.90821492927058770002e-10, r);
-    double q = 1.6059043836821613e-10;                                // 1/13!
-    q = fma(q, r, 2.08767569878681e-09);                              // 1/12!
-    q = fma(q, r, 2.505210838544172e-08);
-    q = fma(q, r, 2.755731922398589e-07);
-    q = fma(q, r, 2.7557319223985893e-06);
-    q = fma(q, r, 2.48015873015873e-05);
-    q = fma(q, r, 1.984126984126984e-04);
-    q = fma(q, r, 1.388888888888889e-03);
-    q = fma(q, r, 8.333333333333333e-03);
-    q = fma(q, r, 4.1666666666666664e-02);
-    q = fma(q, r, 1.6666666666666666e-01);
-    q = fma(q, r, 0.5);
-    q = fma(q, r, 1.0);
-    q = fma(q, r, 1.0);
-    const int k = __double2loint(t);
-    return q * __hiloint2double((k + 1023) << 20, 0);
-}
-// P^1.1 and P^1.4 (Eq 29c-d) for P > 0 without log / pow: z ~ P^-0.1 from the fp32 units,
-// two Newton steps z <- z (1 + (1 - P z^10)/10) (error 5.5 e^2 per step), u = P z^9 ~ P^0.1
-// with one quasi-Newton step on u^10 = P, then P^1.1 = P u, P^1.4 = P u^4.  P <= 0 gives NaN.
-__device__ __forceinline__ void pow_11_14(double P, double& p11, double& p14)
-{
-    double z = (double)__powf((float)P, -0.1f);
-#pragma unroll
-    for (int it = 0; it < 2; ++it) {
-        const double z2 = z * z, z4 = z2 * z2, z5 = z4 * z, z10 = z5 * z5;
-        z = fma(0.1 * z, fma(-P, z10, 1.0), z);
-    }
-    const double z2 = z * z, z4 = z2 * z2, z9 = z4 * z4 * z;
-    double u = P * z9;
-    const double u2 = u * u, u4 = u2 * u2, u5 = u4 * u;
-    u = fma(-0.1 * z9, fma(u5, u5, -P), u);
-    const double v2 = u * u;
-    p11 = P * u; p14 = P * (v2 * v2);
-}
 #endif
 
 // x <-> y swap of the 14 moments (primitive or conserved); an involution.
@@ -145,6 +96,7 @@ struct Params {               // per-solver constants, passed by value to the ke
     double inv_tau_const;     // MM_TAU_CONST: 1/tau
     int tau_model, limiter, shared_limiter, flux;
     int nx, ny, pitch, rows;  // padded array: rows x pitch doubles per moment, interior at (+2,+2)
+    const double* ab;         // table of the functions a(P*), b(P*) of Eq 29c-d (AbTable below)
 };
 
 __device__ __forceinline__ double clamp_sigma(double s, double lim)
@@ -171,12 +123,12 @@ struct PsiMin {
     double n = 0.5, d = 1.0;
     __device__ __forceinline__ void add(int lim, double dm, double dp)
     {
-        const double prod = dm * dp;
+        const double prod = dm * dp, am = fabs(dm), ap = fabs(dp);
         double nk, dk;
-        if (lim == 1) { nk = fmin(fabs(dm), fabs(dp)); dk = fabs(dm) + fabs(dp); }
+        if (lim == 1) { nk = am < ap ? am : ap; dk = am + ap; }
         else { nk = prod; dk = dm * dm + dp * dp; }
         const bool pos = prod > 0.0;
-        const bool flat = (dm == 0.0) && (dp == 0.0);
+        const bool flat = lim == 1 ? dk == 0.0 : (dm == 0.0) && (dp == 0.0);
         nk = pos ? nk : (flat ? 0.5 : 0.0);
         dk = pos ? dk : 1.0;
         if (nk * d < n * dk) { n = nk; d = dk; }
@@ -448,17 +400,84 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
     return t;
 }
 
+// ---- a(P*) = 1.4 P*^1.1 exp(-P*^2) and b(P*) = 0.9 P* exp(-P*^1.4 / 2) of Eq 29c-d (L397-399)
+// They depend on the single variable P* = p_dd in (0, 3] and cost a pow and two exp per call,
+// six calls per cell update.  They are tabulated once per solver (k_ab_table, on the device, from
+// the formulas with libm pow / exp) as degree-13 Chebyshev interpolants re-expanded in powers of
+// the local coordinate t in [-1, 1], on 40 intervals read off the bits of P*:
+//   [2^-5, 2): 4 per octave, [2^e (1 + j/4), 2^e (1 + (j+1)/4));   [2, 4): 16 of width 1/8.
+// The branch point P* = 0 is at least 9 half-widths from every interval's centre (interpolation
+// error < 18^-14) and exp(-P*^2) varies by less than e^(+-1/2) over a half-width (its Chebyshev
+// coefficients fall below 1e-17 by degree 13); what remains is the round-off of 13 FMAs.
+// mm_selftest_fastmath measures it against the direct formulas.  Outside [2^-5, 4) and for NaN
+// the direct formulas are used.
+struct AbTable {
+    static constexpr int kLow = 24, kHigh = 16, kIntervals = kLow + kHigh, kDeg = 13;
+    static constexpr int kStride = 2 * (kDeg + 1);                  // a[14], b[14], highest power first
+    static constexpr int kDoubles = kIntervals * kStride;
+    static constexpr int kHiMin = (1023 - 5) << 20;                 // hi word of 2^-5, 2 and 4
+    static constexpr int kHiTwo = (1023 + 1) << 20, kHiMax = (1023 + 2) << 20;
+    // interval i: lower edge and 1 / half-width
+    __host__ __device__ static double lower(int i)
+    {
+        return i < kLow ? (1.0 + 0.25 * (i & 3)) * (1.0 / 32.0) * (double)(1 << (i >> 2)) : 2.0 + 0.125 * (i - kLow);
+    }
+    __host__ __device__ static double inv_half(int i)
+    {
+        return i < kLow ? 256.0 / (double)(1 << (i >> 2)) : 16.0;
+    }
+};
+#ifndef MM_OPCOUNT_HOST
+__device__ __noinline__ void ab_direct(double P, double* a, double* b)
+{
+    *a = 1.4 * pow(P, 1.1) * exp(-(P * P));
+    *b = 0.9 * P * exp(-0.5 * pow(P, 1.4));
+}
+__device__ __forceinline__ void ab_eval(const double* __restrict__ tab, double P, double& a, double& b)
+{
+    const int hi = __double2hiint(P);
+    if (hi >= AbTable::kHiMin && hi < AbTable::kHiMax) {
+        const bool up = hi >= AbTable::kHiTwo;
+        const int idx = up ? AbTable::kLow + ((hi >> 16) & 15) : (hi >> 18) - (AbTable::kHiMin >> 18);
+        const double lo = __hiloint2double(hi & (up ? 0xFFFF0000 : 0xFFFC0000), 0);
+        // 1 / half-width: 16 on [2, 4), 2^(3 - e) on [2^e, 2^(e+1))
+        const double ih = __hiloint2double(up ? 0x40300000 : (2049 << 20) - (hi & 0x7FF00000), 0);
+        const double t = fma(P - lo, ih, -1.0);
+        const double* c = tab + idx * AbTable::kStride;
+        double qa = c[0], qb = c[AbTable::kDeg + 1];
+#pragma unroll
+        for (int i = 1; i <= AbTable::kDeg; ++i) {
+            qa = fma(qa, t, c[i]);
+            qb = fma(qb, t, c[AbTable::kDeg + 1 + i]);
+        }
+        a = qa; b = qb;
+    } else {
+        ab_direct(P, &a, &b);
+    }
+}
+#else
+__forceinline__ void ab_eval(const double* tab, double P, double& a, double& b)
+{   // same operations, counted: local coordinate + two degree-13 Horner evaluations
+    const double t = (P - 1.0) * 32.0 - 1.0;
+    double qa = tab[0], qb = tab[AbTable::kDeg + 1];
+    for (int i = 1; i <= AbTable::kDeg; ++i) {
+        qa = qa * t + tab[i];
+        qb = qb * t + tab[AbTable::kDeg + 1 + i];
+    }
+    a = qa; b = qb;
+}
+#endif
+
 // Eq 29a-e (L393-403): lambda*_max and -lambda*_min along one direction given P* = p_dd, the
 // heat flux along (hd) and across (qt2 = sum of squares of the other two), sigma_bar terms.
-// P^1.1 and P^1.4 come from pow_11_14 (no log / pow), the exponentials from exp_neg; Y = B + E^2 - 2 E sqrt(B)
+// a(P*), b(P*) come from the table (ab_eval); Y = B + E^2 - 2 E sqrt(B)
 // is evaluated as (sqrt(B) - E)^2; the radicand is floored at 0 (R6).
-__device__ __forceinline__ void ws14_dir(double Pdd, double hd, double qt2, const SbTerms& t,
-                                         double& lam_max, double& lam_min_neg)
+__device__ __forceinline__ void ws14_dir(const double* __restrict__ ab, double Pdd, double hd,
+                                         double qt2, const SbTerms& t, double& lam_max,
+                                         double& lam_min_neg)
 {
-    double p11, p14;
-    pow_11_14(Pdd, p11, p14);
-    const double a = 1.4 * p11 * exp_neg(-(Pdd * Pdd));
-    const double b = 0.9 * Pdd * exp_neg(-0.5 * p14);
+    double a, b;
+    ab_eval(ab, Pdd, a, b);
     const double C = fsqrt((3.0 - 3.0 * t.sb) * Pdd);
     const double E = 0.8 * C;
     const double sY = t.sqB - E;
@@ -479,7 +498,7 @@ __device__ __forceinline__ void wavespeed14_x(const Params& p, const Star14<Z>& 
                                               const SbTerms& t, double ux, double& lmin, double& lmax)
 {
     double a, b;
-    ws14_dir(s.pxx, s.hx, s.hy * s.hy + s.hz * s.hz, t, a, b);
+    ws14_dir(p.ab, s.pxx, s.hx, s.hy * s.hy + s.hz * s.hz, t, a, b);
     const double kc = p.ws_scale * s.c;
     lmax = ux + kc * a; lmin = ux - kc * b;
 }
@@ -489,7 +508,7 @@ __device__ __forceinline__ void wavespeed14_y(const Params& p, const Star14<Z>& 
                                               const SbTerms& t, double uy, double& lmin, double& lmax)
 {
     double a, b;
-    ws14_dir(s.pyy, s.hy, s.hx * s.hx + s.hz * s.hz, t, a, b);
+    ws14_dir(p.ab, s.pyy, s.hy, s.hx * s.hx + s.hz * s.hz, t, a, b);
     const double kc = p.ws_scale * s.c;
     lmax = uy + kc * a; lmin = uy - kc * b;
 }

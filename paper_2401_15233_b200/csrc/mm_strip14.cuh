@@ -7,7 +7,8 @@
 //   cons  [2][NV][34]  conserved rows in flight: filled by cp.async one row ahead of use, so the
 //                      HBM latency of row r+2 hides behind the work on row r at no register cost;
 //   acc   [NV][32]     partial update of the row being assembled;
-//   hsv   [NV][32]     half slopes in y of the previous row (each slope is computed once).
+//   hsv   [NV][32]     half slopes in y of the previous row (each slope is computed once);
+// and per block the 9 KB table of the wave-speed functions a(P*), b(P*) (mm_physics.cuh).
 // Every interface is evaluated in one form: the lane holds a centre cell C with its two
 // neighbours M and P along the direction, computes C's limited half slope h (a3), obtains the
 // half slope hM of M from the lane / row that computed it, and evaluates the interface M|C
@@ -29,9 +30,9 @@ namespace mm {
 constexpr int kSW = 30;                 // cells per strip
 constexpr int kRW = 34;                 // staged cells per row: 2 + 30 + 2
 #ifndef MM_STRIP_WPB
-#define MM_STRIP_WPB 2
+#define MM_STRIP_WPB 1
 #endif
-constexpr int kStripWPB = MM_STRIP_WPB; // warps per block (a container only)
+constexpr int kStripWPB = MM_STRIP_WPB; // warps per block (a block is only a container of warps)
 
 // Moments carried by a kernel variant and their compact numbering.
 template <bool ZS>
@@ -61,8 +62,12 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // Work decomposition: item = (strip, chunk); chunk c covers rows [c ny / nchunks, (c+1) ny / nchunks).
 template <bool ZS, int MINB>
+#ifdef MM_MAXNREG
+__global__ void __maxnreg__(MM_MAXNREG)
+#else
 __global__ void __launch_bounds__(32 * kStripWPB, MINB)
-k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl,
+#endif
+k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl,
                int slot_next, int nstrips, int nchunks)
 {
     using Z = typename std::conditional<ZS, zero_t, double>::type;
@@ -70,6 +75,12 @@ k_step14_strip(Params p, const double* __restrict__ Uin, double* __restrict__ Uo
     constexpr int NM = 14, NV = M::NV, RS = NV * kRW;          // RS: doubles per staged row
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // the block's copy of the a(P*), b(P*) table (Eq 29c-d), behind the warps' buffers
+    double* tab = smem + kStripWPB * M::warp_smem_doubles;
+    for (int i = threadIdx.x; i < AbTable::kDoubles; i += 32 * kStripWPB) tab[i] = pg.ab[i];
+    __syncthreads();
+    Params p = pg;
+    p.ab = tab;
     const int item = blockIdx.x * kStripWPB + warp;
     if (item >= nstrips * nchunks) return;
     const int strip = item % nstrips, chunk = item / nstrips;

@@ -121,10 +121,11 @@ def mm_measure_fp64_peak(repeats: int = 5, stream=None) -> float:
 
 
 def mm_selftest_fastmath(n: int = 1 << 22, stream=None):
-    """Max relative error (units of 2^-53) of the library's rcp, sqrt, exp, P^1.1|P^1.4 (mm.h)."""
+    """Max relative error (units of 2^-53) of the library's rcp, sqrt and tabulated a(P*), b(P*)
+    (include/mm.h)."""
     import torch
     st = stream if stream is not None else torch.cuda.current_stream()
-    out = (C.c_double * 4)()
+    out = (C.c_double * 3)()
     _check(lib().mm_selftest_fastmath(C.c_void_p(st.cuda_stream), n, out))
     return tuple(out)
 

@@ -196,11 +196,13 @@ def test_fast_path_selection(mm):
 
 
 def test_fastmath_accuracy(mm):
-    """The branch-free reciprocal, square root, exp and P^1.1 / P^1.4 of the CUDA path against
-    IEEE division / sqrt and libm over 4 M arguments, in units of 2^-53 relative."""
-    e_rcp, e_sqrt, e_exp, e_pow = mm.mm_selftest_fastmath(1 << 22)
-    assert 0.0 < e_rcp <= 2.0 and 0.0 <= e_sqrt <= 2.0, (e_rcp, e_sqrt)
-    assert 0.0 < e_exp <= 4.0 and 0.0 < e_pow <= 16.0, (e_exp, e_pow)
+    """The branch-free reciprocal and square root of the CUDA path against IEEE division / sqrt,
+    and the tabulated wave-speed functions a(P*), b(P*) (Eq 29c-d) against the direct formulas with
+    libm pow / exp, over 4 M arguments; in units of 2^-53 relative.  The direct formula itself
+    is only good to ~P*^2 units (rounding of P*^2 in the exponent), hence the wider last bound."""
+    e_rcp, e_sqrt, e_ab = mm.mm_selftest_fastmath(1 << 22)
+    assert 0.0 < e_rcp <= 2.0 and 0.0 < e_sqrt <= 2.5, (e_rcp, e_sqrt)
+    assert 0.0 < e_ab <= 40.0, e_ab
 
 
 def test_smooth14_transmissive(mm, mmo):
