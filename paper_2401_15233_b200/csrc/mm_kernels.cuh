@@ -91,7 +91,7 @@ __device__ __forceinline__ void cell_rate(const Params& p, const double (&U)[NM]
         cons2prim14<Z>(U, W);
         double sx, sy;
         ok = cell_speeds14<Z>(p, W, sx, sy);
-        rate = fmax(sx / p.dx, sy / p.dy); speed = fmax(sx, sy);
+        rate = dmax(sx / p.dx, sy / p.dy); speed = dmax(sx, sy);
     }
     // finite test: NaN or Inf fail (x - x != 0)
     if (!ok || !(rate - rate == 0.0)) { bad = 1; rate = 0.0; speed = 0.0; }
@@ -279,11 +279,11 @@ __device__ __forceinline__ void interface_flux5(const Params& p, const double* _
         Wam[k] = q[-2]; Wa[k] = q[-1]; Wb[k] = q[0]; Wbp[k] = q[1];
     }
     if (p.limiter != 0 && p.shared_limiter) {
-        PsiMin ma, mb;
+        PsiShared ma, mb;
 #pragma unroll
         for (int k = 0; k < NM; ++k) {
-            ma.add(p.limiter, Wa[k] - Wam[k], Wb[k] - Wa[k]);
-            mb.add(p.limiter, Wb[k] - Wa[k], Wbp[k] - Wb[k]);
+            ma.add(p.limiter, Wa[k] - Wam[k], Wb[k] - Wa[k], (Wa[k] - Wam[k]) + (Wb[k] - Wa[k]));
+            mb.add(p.limiter, Wb[k] - Wa[k], Wbp[k] - Wb[k], (Wb[k] - Wa[k]) + (Wbp[k] - Wb[k]));
         }
         const double qa = 0.25 * ma.psi(), qb = 0.25 * mb.psi();
 #pragma unroll
@@ -431,7 +431,7 @@ __global__ void k_ab_table(double* __restrict__ tab)
         for (int j = 0; j < N; ++j) { m[j] = fma(c[k], Tn[j], m[j]); Tkm1[j] = Tk[j]; Tk[j] = Tn[j]; }
     }
     double* out = tab + i * AbTable::kStride;
-    for (int j = 0; j < N; ++j) out[f * N + j] = m[N - 1 - j];
+    for (int j = 0; j < N; ++j) out[2 * j + f] = m[N - 1 - j];
 }
 
 // max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x), and of the

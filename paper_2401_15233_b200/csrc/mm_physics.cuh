@@ -49,13 +49,31 @@ __host__ __device__ __forceinline__ void zadd(double&, zero_t) {}
 // fsqrt(x) = 0 for |x| < 1e-290; negative or NaN arguments give NaN.  rcp is only applied to
 // well-scaled arguments (densities, pressures, O(1) determinants, wave-speed differences).
 // -DMM_EXACT_MATH restores IEEE div/sqrt.
+// dmin / dmax: one compare and one select (fmin / fmax cost six instructions for their NaN rules);
+// like fmin / fmax they return the second argument when the first is NaN.
 #ifdef MM_OPCOUNT_HOST
 __forceinline__ double rcp(double x) { return 1.0 / x; }
 __forceinline__ double fsqrt(double x) { return sqrt(x); }
+__forceinline__ double rsqrt_nr(double x) { return 1.0 / sqrt(x); }
+__forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 #elif defined(MM_EXACT_MATH)
 __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
 __device__ __forceinline__ double fsqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ double rsqrt_nr(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 #else
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+// 1/sqrt(x) for normal x > 0
+__device__ __forceinline__ double rsqrt_nr(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-(x * y), y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
+}
 __device__ __forceinline__ double rcp(double x)
 {
     double r;
@@ -102,7 +120,7 @@ struct Params {               // per-solver constants, passed by value to the ke
 __device__ __forceinline__ double clamp_sigma(double s, double lim)
 {
     // sigma_bar = min(max(sigma, sigma_lim), 1)  (L163, L512; upper clamp: DESIGN.md R5)
-    return fmin(fmax(s, lim), 1.0);
+    return dmin(dmax(s, lim), 1.0);
 }
 
 // ------------------------------------------------------------------ limiter (L262-266)
@@ -114,29 +132,28 @@ __device__ __forceinline__ double limited_slope(int lim, double dm, double dp)
     return dm * dp * (dm + dp) / (dm * dm + dp * dp);     // IEEE: differences may be subnormal
 }
 
-// Shared, most stringent limiter value (L266) over a set of variables, without a division per
-// variable: psi_k = 2 n_k / d_k with (n_k, d_k) = (min(|dm|,|dp|), |dm|+|dp|) for minmod and
-// (dm dp, dm^2+dp^2) for van Albada when dm dp > 0, psi_k = 0 otherwise; a variable with
-// dm = dp = 0 imposes nothing (R14).  The running minimum is kept as a fraction
-// n/d and compared by cross-multiplication; psi = 2 n / d is formed once at the end.
-struct PsiMin {
-    double n = 0.5, d = 1.0;
-    __device__ __forceinline__ void add(int lim, double dm, double dp)
+// Shared, most stringent limiter value (L266) over a set of variables, without a division or a
+// sign test per variable.  For dm dp > 0 both limiter functions are one minus a ratio,
+//   minmod      2 min(|dm|,|dp|)/(|dm|+|dp|) = 1 - |dm - dp| / |dm + dp|,
+//   van Albada  2 dm dp / (dm^2 + dp^2)       = 1 - (dm - dp)^2 / (dm^2 + dp^2),
+// and for dm dp <= 0 that ratio is >= 1, so psi = max(0, 1 - max_k N_k / D_k) covers every case;
+// a variable with dm = dp = 0 has N = D = 0 and never wins the comparison, i.e. imposes nothing
+// (R14).  The running maximum is kept as a fraction and compared by cross-multiplication;
+// one IEEE division per slope forms psi.  `s` = dm + dp is shared with the slope itself.
+struct PsiShared {
+    double n = 0.0, d = 1.0;
+    __device__ __forceinline__ void add(int lim, double dm, double dp, double s)
     {
-        const double prod = dm * dp, am = fabs(dm), ap = fabs(dp);
         double nk, dk;
-        if (lim == 1) { nk = am < ap ? am : ap; dk = am + ap; }
-        else { nk = prod; dk = dm * dm + dp * dp; }
-        const bool pos = prod > 0.0;
-        const bool flat = lim == 1 ? dk == 0.0 : (dm == 0.0) && (dp == 0.0);
-        nk = pos ? nk : (flat ? 0.5 : 0.0);
-        dk = pos ? dk : 1.0;
-        if (nk * d < n * dk) { n = nk; d = dk; }
+        if (lim == 1) { nk = fabs(dm - dp); dk = fabs(s); }
+        else { const double t = dm - dp; nk = t * t; dk = dm * dm + dp * dp; }
+        if (nk * d > n * dk) { n = nk; d = dk; }
     }
-    // IEEE division (one per slope): psi is then the correctly rounded 2 n_k / d_k of the
-    // winning variable, which keeps the limiter free of extra round-off -- the shared-psi
-    // scheme amplifies round-off in psi by ~1e3 over 30 steps (R24)
-    __device__ __forceinline__ double psi() const { return (2.0 * n) / d; }
+    __device__ __forceinline__ double psi() const
+    {
+        const double r = n / d;
+        return r < 1.0 ? 1.0 - r : 0.0;
+    }
 };
 
 // ============================================================================ 5-moment
@@ -394,8 +411,9 @@ struct SbTerms { double sb, ss, isb, B, sqB; };
 __device__ __forceinline__ SbTerms sb_terms(double sb)
 {
     SbTerms t;
-    t.sb = sb; t.ss = fsqrt(sb); t.isb = rcp(sb);
-    t.B = 5.0 - 4.0 * t.ss + fsqrt(fmax(10.0 - 16.0 * t.ss + 6.0 * sb, 0.0));   // Eq 29e
+    const double y = rsqrt_nr(sb);                     // sb >= sigma_lim > 0
+    t.sb = sb; t.ss = sb * y; t.isb = y * y;
+    t.B = 5.0 - 4.0 * t.ss + fsqrt(dmax(10.0 - 16.0 * t.ss + 6.0 * sb, 0.0));   // Eq 29e
     t.sqB = fsqrt(t.B);
     return t;
 }
@@ -413,7 +431,7 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
 // the direct formulas are used.
 struct AbTable {
     static constexpr int kLow = 24, kHigh = 16, kIntervals = kLow + kHigh, kDeg = 13;
-    static constexpr int kStride = 2 * (kDeg + 1);                  // a[14], b[14], highest power first
+    static constexpr int kStride = 2 * (kDeg + 1);                  // (a_i, b_i) pairs, highest power first
     static constexpr int kDoubles = kIntervals * kStride;
     static constexpr int kHiMin = (1023 - 5) << 20;                 // hi word of 2^-5, 2 and 4
     static constexpr int kHiTwo = (1023 + 1) << 20, kHiMax = (1023 + 2) << 20;
@@ -443,14 +461,15 @@ __device__ __forceinline__ void ab_eval(const double* __restrict__ tab, double P
         // 1 / half-width: 16 on [2, 4), 2^(3 - e) on [2^e, 2^(e+1))
         const double ih = __hiloint2double(up ? 0x40300000 : (2049 << 20) - (hi & 0x7FF00000), 0);
         const double t = fma(P - lo, ih, -1.0);
-        const double* c = tab + idx * AbTable::kStride;
-        double qa = c[0], qb = c[AbTable::kDeg + 1];
+        const double2* c = reinterpret_cast<const double2*>(tab + idx * AbTable::kStride);
+        double2 q = c[0];
 #pragma unroll
         for (int i = 1; i <= AbTable::kDeg; ++i) {
-            qa = fma(qa, t, c[i]);
-            qb = fma(qb, t, c[AbTable::kDeg + 1 + i]);
+            const double2 ci = c[i];
+            q.x = fma(q.x, t, ci.x);
+            q.y = fma(q.y, t, ci.y);
         }
-        a = qa; b = qb;
+        a = q.x; b = q.y;
     } else {
         ab_direct(P, &a, &b);
     }
@@ -459,10 +478,10 @@ __device__ __forceinline__ void ab_eval(const double* __restrict__ tab, double P
 __forceinline__ void ab_eval(const double* tab, double P, double& a, double& b)
 {   // same operations, counted: local coordinate + two degree-13 Horner evaluations
     const double t = (P - 1.0) * 32.0 - 1.0;
-    double qa = tab[0], qb = tab[AbTable::kDeg + 1];
+    double qa = tab[0], qb = tab[1];
     for (int i = 1; i <= AbTable::kDeg; ++i) {
-        qa = qa * t + tab[i];
-        qb = qb * t + tab[AbTable::kDeg + 1 + i];
+        qa = qa * t + tab[2 * i];
+        qb = qb * t + tab[2 * i + 1];
     }
     a = qa; b = qb;
 }
@@ -473,7 +492,7 @@ __forceinline__ void ab_eval(const double* tab, double P, double& a, double& b)
 // a(P*), b(P*) come from the table (ab_eval); Y = B + E^2 - 2 E sqrt(B)
 // is evaluated as (sqrt(B) - E)^2; the radicand is floored at 0 (R6).
 __device__ __forceinline__ void ws14_dir(const double* __restrict__ ab, double Pdd, double hd,
-                                         double qt2, const SbTerms& t, double& lam_max,
+                                         double qt, double qt2, const SbTerms& t, double& lam_max,
                                          double& lam_min_neg)
 {
     double a, b;
@@ -484,10 +503,9 @@ __device__ __forceinline__ void ws14_dir(const double* __restrict__ ab, double P
     const double pref = (a * t.sb + b) * (0.5 * t.isb);
     const double sC = 0.8 * t.sb * C;
     const double cst = 4.0 * t.sb * t.sb * (sY * sY) + 0.1 * qt2;
-    const double qt = fsqrt(qt2);                                    // Eq 28, qtilde >= 0 (R7)
     const double alpha = (0.6 * Pdd - 0.38) * Pdd + 0.35;            // Eq 29b
     const double zp = hd + alpha * qt, zm = -hd + alpha * qt;        // Eq 30: q_d -> -q_d
-    const double rp = fmax(zp * zp - zp * sC + cst, 0.0), rm = fmax(zm * zm - zm * sC + cst, 0.0);
+    const double rp = dmax(zp * zp - zp * sC + cst, 0.0), rm = dmax(zm * zm - zm * sC + cst, 0.0);
     lam_max = pref * (zp + fsqrt(rp)) + E;
     lam_min_neg = pref * (zm + fsqrt(rm)) + E;
 }
@@ -497,8 +515,10 @@ template <class Z>
 __device__ __forceinline__ void wavespeed14_x(const Params& p, const Star14<Z>& s,
                                               const SbTerms& t, double ux, double& lmin, double& lmax)
 {
-    double a, b;
-    ws14_dir(p.ab, s.pxx, s.hx, s.hy * s.hy + s.hz * s.hz, t, a, b);
+    double a, b, qt;                                                 // Eq 28: qtilde >= 0 (R7)
+    const double qt2 = s.hy * s.hy + s.hz * s.hz;
+    if constexpr (std::is_same<Z, zero_t>::value) qt = fabs(s.hy); else qt = fsqrt(qt2);
+    ws14_dir(p.ab, s.pxx, s.hx, qt, qt2, t, a, b);
     const double kc = p.ws_scale * s.c;
     lmax = ux + kc * a; lmin = ux - kc * b;
 }
@@ -507,8 +527,10 @@ template <class Z>
 __device__ __forceinline__ void wavespeed14_y(const Params& p, const Star14<Z>& s,
                                               const SbTerms& t, double uy, double& lmin, double& lmax)
 {
-    double a, b;
-    ws14_dir(p.ab, s.pyy, s.hy, s.hx * s.hx + s.hz * s.hz, t, a, b);
+    double a, b, qt;
+    const double qt2 = s.hx * s.hx + s.hz * s.hz;
+    if constexpr (std::is_same<Z, zero_t>::value) qt = fabs(s.hx); else qt = fsqrt(qt2);
+    ws14_dir(p.ab, s.pyy, s.hy, qt, qt2, t, a, b);
     const double kc = p.ws_scale * s.c;
     lmax = uy + kc * a; lmin = uy - kc * b;
 }
@@ -632,9 +654,9 @@ __device__ __forceinline__ bool cell_speeds14(const Params& p, const double (&W)
     const SbTerms t = sb_terms(clamp_sigma(s.sigma, p.sigma_lim));
     double a, b;
     wavespeed14_x<Z>(p, s, t, W[1], a, b);
-    sx = fmax(fabs(a), fabs(b));
+    sx = dmax(fabs(a), fabs(b));
     wavespeed14_y<Z>(p, s, t, W[2], a, b);
-    sy = fmax(fabs(a), fabs(b));
+    sy = dmax(fabs(a), fabs(b));
     return true;
 }
 

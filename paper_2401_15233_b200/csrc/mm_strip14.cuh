@@ -178,18 +178,26 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restri
                     }
                 } else {
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) { Wm[k] = 1.0; Wc[k] = 1.0; Wp[k] = 1.0; }
+                    for (int k = 0; k < NV; ++k) {   // idle lane: a unit Maxwellian (swap-invariant)
+                        const int m = M::full(k);
+                        const double v = (m == 0 || m == 4 || m == 7 || m == 9) ? 1.0 : (m == 13 ? 15.0 : 0.0);
+                        Wm[k] = v; Wc[k] = v; Wp[k] = v;
+                    }
                 }
                 if (p.limiter == 0) {
 #pragma unroll
                     for (int k = 0; k < NV; ++k) h[k] = 0.0;
                 } else if (p.shared_limiter) {
-                    PsiMin pm;
+                    PsiShared pm;
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) pm.add(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
+                    for (int k = 0; k < NV; ++k) {
+                        const double dm = Wc[k] - Wm[k], dp = Wp[k] - Wc[k];
+                        h[k] = dm + dp;
+                        pm.add(p.limiter, dm, dp, h[k]);
+                    }
                     const double q = 0.25 * pm.psi();
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) h[k] = q * ((Wc[k] - Wm[k]) + (Wp[k] - Wc[k]));
+                    for (int k = 0; k < NV; ++k) h[k] = q * h[k];
                 } else {
 #pragma unroll
                     for (int k = 0; k < NV; ++k)
@@ -218,14 +226,14 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restri
                 eval_face14<Z>(p, WL, FL, UL, lminL, lmaxL);
                 eval_face14<Z>(p, WR, FR, UR, lminR, lmaxR);
                 if (p.flux == 1) {
-                    const double S = fmax(fmax(fabs(lminL), fabs(lmaxL)), fmax(fabs(lminR), fabs(lmaxR)));
+                    const double S = dmax(dmax(fabs(lminL), fabs(lmaxL)), dmax(fabs(lminR), fabs(lmaxR)));
 #pragma unroll
                     for (int k = 0; k < NV; ++k) {
                         const int m = M::full(k);
                         Fh[k] = 0.5 * (FL[m] + FR[m]) - 0.5 * S * (UR[m] - UL[m]);
                     }
                 } else {
-                    const double SL = fmin(fmin(lminL, lminR), 0.0), SR = fmax(fmax(lmaxL, lmaxR), 0.0);
+                    const double SL = dmin(dmin(lminL, lminR), 0.0), SR = dmax(dmax(lmaxL, lmaxR), 0.0);
                     const double inv = rcp(SR - SL), SLR = SL * SR;
 #pragma unroll
                     for (int k = 0; k < NV; ++k) {
@@ -257,7 +265,7 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restri
                         }
                         double rr, ss;
                         cell_rate<NM, Z>(p, Un, rr, ss, bad);
-                        rate = fmax(rate, rr); speed = fmax(speed, ss);
+                        rate = dmax(rate, rr); speed = dmax(speed, ss);
                     }
                     if (r < y1) {
 #pragma unroll

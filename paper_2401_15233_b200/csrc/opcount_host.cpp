@@ -54,17 +54,19 @@ template <int NM>
 static void half_slope(const Params& p, const cnt (&Wm)[NM], const cnt (&Wc)[NM], const cnt (&Wp)[NM],
                        cnt (&h)[NM], bool zs)
 {
-    PsiMin pm;
+    PsiShared pm;
     for (int k = 0; k < NM; ++k) {
         if (NM == 14 && zs && z_odd(k)) continue;
-        if (p.shared_limiter) pm.add(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
-        else h[k] = 0.5 * limited_slope(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
+        const cnt dm = Wc[k] - Wm[k], dp = Wp[k] - Wc[k];
+        h[k] = dm + dp;
+        if (p.shared_limiter) pm.add(p.limiter, dm, dp, h[k]);
+        else h[k] = 0.5 * limited_slope(p.limiter, dm, dp);
     }
     if (p.shared_limiter) {
         const cnt q = 0.25 * pm.psi();
         for (int k = 0; k < NM; ++k) {
             if (NM == 14 && zs && z_odd(k)) continue;
-            h[k] = q * ((Wc[k] - Wm[k]) + (Wp[k] - Wc[k]));
+            h[k] = q * h[k];
         }
     }
 }
