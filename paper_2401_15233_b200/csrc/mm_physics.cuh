@@ -139,7 +139,7 @@ __device__ __forceinline__ double limited_slope(int lim, double dm, double dp)
 // and for dm dp <= 0 that ratio is >= 1, so psi = max(0, 1 - max_k N_k / D_k) covers every case;
 // a variable with dm = dp = 0 has N = D = 0 and never wins the comparison, i.e. imposes nothing
 // (R14).  The running maximum is kept as a fraction and compared by cross-multiplication;
-// one IEEE division per slope forms psi.  `s` = dm + dp is shared with the slope itself.
+// one reciprocal per slope forms psi.  `s` = dm + dp is shared with the slope itself.
 struct PsiShared {
     double n = 0.0, d = 1.0;
     __device__ __forceinline__ void add(int lim, double dm, double dp, double s)
@@ -151,7 +151,8 @@ struct PsiShared {
     }
     __device__ __forceinline__ double psi() const
     {
-        const double r = n / d;
+        // d = 0 or subnormal (dm = -dp, or differences below 1e-300) makes rcp NaN -> psi = 0
+        const double r = n * rcp(d);
         return r < 1.0 ? 1.0 - r : 0.0;
     }
 };
