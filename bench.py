@@ -56,7 +56,7 @@ def peaks() -> dict:
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -67,7 +67,7 @@ class ClockSampler:
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
                  "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -261,8 +261,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--n", type=int, default=2048)
     ap.add_argument("--kn", type=float, default=0.1)
-    ap.add_argument("--ref-n", type=int, default=256, help="grid of the bounded oracle sample")
-    ap.add_argument("--cpu-steps", type=int, default=40)
+    ap.add_argument("--ref-n", type=int, default=512, help="grid of the bounded oracle sample")
+    ap.add_argument("--cpu-steps", type=int, default=250,
+                    help="oracle steps of the cpu_baseline leg (~15 s on 16 cores at 512^2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--general-path", action="store_true",
                     help="forbid the z-symmetric kernel variant (measurement of the general one)")
