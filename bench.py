@@ -102,6 +102,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(x: float, device) -> float:
+    """Device-timed milliseconds -> max over all ranks (replicas finish when the slowest does)."""
+    import torch
+    import torch.distributed as dist
+    if not dist.is_available() or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(world: int, cells: int, steps: int, ms: float) -> float:
+    """Whole-job cell-updates/s: every rank steps its own replica of `cells` cells."""
+    return world * cells * steps / (ms * 1e-3)
+
+
 def workload(n: int, kn: float) -> dict:
     return wl.crossed_jets(n, Kn=kn, perturb=0.01)
 
@@ -186,11 +202,8 @@ def run_gpu(args):
     ms = ev0.elapsed_time(ev1)
     launches = s.launches - l0
     info = s.info()
-    if world > 1:
-        t = torch.tensor([ms], device=f"cuda:{local}", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * cells * K / (ms * 1e-3)
+    ms = max_over_ranks(ms, f"cuda:{local}")
+    value = job_throughput(world, cells, K, ms)
 
     # ---- end to end through the API with HOST buffers: H2D of the state, K steps, D2H of the result
     barrier()
@@ -203,11 +216,8 @@ def run_gpu(args):
     e1.record(s.stream)
     barrier()
     e2e_ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=f"cuda:{local}", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_value = world * cells * K / (e2e_ms * 1e-3)
+    e2e_ms = max_over_ranks(e2e_ms, f"cuda:{local}")
+    e2e_value = job_throughput(world, cells, K, e2e_ms)
     finite = bool(torch.isfinite(U_host).all())
 
     if rank == 0:
