@@ -363,7 +363,7 @@ __device__ __forceinline__ void nondim_sigma14(const double (&W)[14], Star14<Z>&
 {
     const double rho = W[0];
     const double Ph = (W[4] + W[7] + W[9]) * (1.0 / 3.0);
-    const double iP = rcp(Ph), ir = rcp(rho);
+    const double rr = rcp(Ph * rho), iP = rr * rho, ir = rr * Ph;      // one reciprocal for both
     const double c2 = Ph * ir, c = fsqrt(c2);
     s.c = c; s.Ph = Ph;
     s.pxx = W[4] * iP; s.pxy = W[5] * iP; s.pxz = zget<Z>(W[6]) * iP;

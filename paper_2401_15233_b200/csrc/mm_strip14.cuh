@@ -153,36 +153,27 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restri
         const int cs = (r - y0) & 1;
 #pragma unroll 1
         for (int d = 0; d < 2; ++d) {
+            // Lanes without an interface of their own (beyond the strip's last cell / staged column)
+            // take the last valid cell's data, so every lane evaluates a valid state; their
+            // results are never used.
             const double *qm, *qc, *qp;              // plane 0 of the cells M, C, P
-            bool act;
             if (d == 0) {                            // y: C = (row r, cell lane)
-                const double* b = ring + lane + 2;
+                const double* b = ring + min(lane, ncell - 1) + 2;
                 qm = b + sm * RS; qc = b + sc * RS; qp = b + sp * RS;
-                act = cell_ok;
             } else {                                 // x: C = (row r, cell lane-1)
                 if (r < y0 || r == y1) break;
                 __syncwarp();                        // every lane has taken U_r out of cons[cs]
                 load_row(r + 2, cs);
-                qm = ring + sc * RS + lane; qc = qm + 1; qp = qm + 2;
-                act = lane + 2 < ncol;
+                qm = ring + sc * RS + min(lane, ncol - 3); qc = qm + 1; qp = qm + 2;
             }
             // ---- a3: limited half slope of C; face states of the interface M|C
             double WL[NM], WR[NM];
             {
                 double Wm[NV], Wc[NV], Wp[NV], h[NV];
-                if (act) {
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) {
-                        const int o = (d == 0 ? M::cswap(k) : k) * kRW;
-                        Wm[k] = qm[o]; Wc[k] = qc[o]; Wp[k] = qp[o];
-                    }
-                } else {
-#pragma unroll
-                    for (int k = 0; k < NV; ++k) {   // idle lane: a unit Maxwellian (swap-invariant)
-                        const int m = M::full(k);
-                        const double v = (m == 0 || m == 4 || m == 7 || m == 9) ? 1.0 : (m == 13 ? 15.0 : 0.0);
-                        Wm[k] = v; Wc[k] = v; Wp[k] = v;
-                    }
+                for (int k = 0; k < NV; ++k) {
+                    const int o = (d == 0 ? M::cswap(k) : k) * kRW;
+                    Wm[k] = qm[o]; Wc[k] = qc[o]; Wp[k] = qp[o];
                 }
                 if (p.limiter == 0) {
 #pragma unroll
