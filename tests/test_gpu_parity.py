@@ -308,12 +308,14 @@ def test_C3_jets_developed_state(mm, mmo):
     assert_parity(sg.get_state(), so.get_state(), max(1e-9, 10.0 * rel_err(sp.get_state(), so.get_state()).max()))
 
 
-def test_C4_jets_2048_sampled_windows(mm, mmo):
-    """Full bench size, bench launch configuration: after n steps a cell depends only on the
-    (2n)-neighbourhood of its initial data, so the oracle is run on small windows of the same
-    seeded state (transmissive window edges) and compared on the cells no edge can have reached."""
-    n, nsteps, half, margin = 2048, 3, 14, 2 * 3 + 1
-    prob = wl.crossed_jets(n, Kn=0.1, perturb=0.01)
+@pytest.mark.parametrize("n,Kn", [(2048, 0.1), (2048, 1.0), (4096, 0.1)])
+def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn):
+    """Full bench sizes (BASELINE configs[3] and [4]), bench launch configuration: after n steps a
+    cell depends only on the (2n)-neighbourhood of its initial data, so the oracle is run on small
+    windows of the same seeded state (transmissive window edges) and compared on the cells no edge
+    can have reached."""
+    nsteps, half, margin = 3, 14, 2 * 3 + 1
+    prob = wl.crossed_jets(n, Kn=Kn, perturb=0.01)
     sg = mm.Solver.from_problem(prob)
     so_dt = 0.5 * 0.4 * (1.0 / n) / 6.0        # CFL 0.2 against the jets' inflow speed (~5.8)
     sg.step_fixed_dt(nsteps, so_dt)
@@ -322,6 +324,8 @@ def test_C4_jets_2048_sampled_windows(mm, mmo):
     rng = np.random.default_rng(7)
     centres = [(int(a), int(b)) for a, b in rng.integers(half, n - half, size=(6, 2))]
     centres += [(half, int(0.35 * n)), (half, int(0.65 * n)), (half, int(0.5 * n))]   # at the inflow side
+    # across strip boundaries (every 30 cells) and row-chunk boundaries of the launch decomposition
+    centres += [(30 * 20, n * 5 // 17), (30 * 41, n * 9 // 17 + 1), (30 * (n // 30) - 6, n // 2), (n - half, n - half)]
     h = 1.0 / n
     for (ci, cj) in centres:
         i0, j0 = ci - half, cj - half
