@@ -118,8 +118,23 @@ def job_throughput(world: int, cells: int, steps: int, ms: float) -> float:
     return world * cells * steps / (ms * 1e-3)
 
 
+WORKLOADS = {
+    # name: (builder(n, kn), CFL, description)
+    "baseline": (lambda n, kn: wl.crossed_jets(n, Kn=kn, perturb=0.01), 0.4,
+                 "crossed jets {n}x{n}, 14-moment, Kn={kn}, +-1% seeded density perturbation, minmod (shared psi) "
+                 "+ HLL, CFL 0.4 (BASELINE configs[3])"),
+    "paper-crossing": (lambda n, kn: wl.paper_jets(n, two=True), 0.5,
+                       "the paper's collisionless M=5 crossing jets {n}x{n} (PAPER.md L446-470), van Albada "
+                       "(shared psi) + Rusanov, CFL 0.5; SURVEY 8(f) item 1, not the BASELINE metric's workload"),
+    "paper-single": (lambda n, kn: wl.paper_jets(n, two=False), 0.5,
+                     "the paper's collisionless M=5 single jet {n}x{n} (PAPER.md L430-444), van Albada (shared "
+                     "psi) + Rusanov, CFL 0.5; SURVEY 8(f) item 1, not the BASELINE metric's workload"),
+}
+WORKLOAD = "baseline"
+
+
 def workload(n: int, kn: float) -> dict:
-    return wl.crossed_jets(n, Kn=kn, perturb=0.01)
+    return WORKLOADS[WORKLOAD][0](n, kn)
 
 
 def time_oracle(n: int, kn: float, steps: int, warmup: int = 0, nthreads: int = 0):
@@ -148,8 +163,8 @@ def run_reference(args):
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1),
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic", "gpu_launches": 0,
-           "config": {"workload": f"crossed jets 2048x2048 Kn={args.kn} (BASELINE configs[3]); "
-                                  f"oracle timed on a bounded {n}x{n} sample of it"},
+           "config": {"workload": WORKLOADS[WORKLOAD][2].format(n=args.n, kn=args.kn)
+                                  + f"; oracle timed on a bounded {n}x{n} sample of it"},
            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out), flush=True)
@@ -237,9 +252,8 @@ def run_gpu(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"crossed jets {n}x{n}, 14-moment, Kn={args.kn}, +-1% seeded density "
-                                   f"perturbation, minmod (shared psi) + HLL, CFL {CFL} (BASELINE configs[3])",
-                       "cells": cells, "l2": "inputs larger than L2 (2 x 470 MB state copies)",
+            "config": {"workload": WORKLOADS[WORKLOAD][2].format(n=n, kn=args.kn),
+                       "cells": cells, "l2": f"inputs larger than L2 (2 x {nbytes_state / 1e6:.0f} MB state copies)",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "t_end": info["t"], "state_finite": finite},
             "clocks": clk.summary(),
@@ -275,9 +289,14 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=250,
                     help="oracle steps of the cpu_baseline leg (~15 s on 16 cores at 512^2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="baseline", choices=sorted(WORKLOADS),
+                    help="baseline = BASELINE.json configs[3] (the metric); paper-* = the paper's own jet cases")
     ap.add_argument("--general-path", action="store_true",
                     help="forbid the z-symmetric kernel variant (measurement of the general one)")
     args = ap.parse_args()
+    global WORKLOAD, CFL
+    WORKLOAD = args.workload
+    CFL = WORKLOADS[WORKLOAD][1]
     if args.impl == "reference":
         run_reference(args)
     else:

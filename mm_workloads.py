@@ -115,6 +115,30 @@ def crossed_jets(n: int = 512, Kn: float = 1.0, perturb: float = 0.0, mach: floa
     return _problem(SYS14, n, n, (0.0, 1.0, 0.0, 1.0), col, bcs, W0, **options)
 
 
+def paper_jets(n: int = 1200, two: bool = True, Kn=None, mach: float = 5.0, rho_bg: float = 1e-5, **options):
+    """The paper's own jet cases in its recommended robust configuration (PAPER.md L426-434, L446-470;
+    SURVEY section 8(f) item 1), non-dimensional: unit square, jets of width L/7 centred on the
+    left side (directed +x) and, if `two`, on the bottom side (directed +y, crossing at a right
+    angle), rho_jet = T = 1, Mach `mach` with a = sqrt(5/3 R T), background rho_bg = 1e-5 held on
+    the rest of those sides, the other sides transmissive; collisionless unless Kn is given
+    (Kn based on the jet width, L474).  Rusanov flux (L258), van Albada limiter with one shared
+    psi (L262-266), sigma_lim = 1e-4 (L442); the paper's Courant number is 0.5 (L434)."""
+    options.setdefault("shared_limiter", 1)
+    options.setdefault("limiter", LIM_VANALBADA)
+    options.setdefault("flux", FLUX_RUSANOV)
+    speed = mach * math.sqrt(5.0 / 3.0)
+    lo, hi = 0.5 - 1.0 / 14.0, 0.5 + 1.0 / 14.0
+    jet_x = maxwellian(SYS14, 1.0, (speed, 0.0, 0.0), 1.0)
+    jet_y = maxwellian(SYS14, 1.0, (0.0, speed, 0.0), 1.0)
+    bg = maxwellian(SYS14, rho_bg, (0.0, 0.0, 0.0), 1.0)
+    W0 = maxwellian(SYS14, np.full((n, n), rho_bg), (0.0, 0.0, 0.0), 1.0)
+    col = dict(model=TAU_KN, Kn=Kn, L_ref=1.0 / 7.0, rho_ref=1.0) if Kn is not None else dict(model=TAU_NONE)
+    ylo = dict(type=BC_DIRICHLET, bands=[(lo, hi, jet_y)], default=bg) if two else dict(type=BC_TRANSMISSIVE)
+    bcs = [dict(type=BC_DIRICHLET, bands=[(lo, hi, jet_x)], default=bg), dict(type=BC_TRANSMISSIVE),
+           ylo, dict(type=BC_TRANSMISSIVE)]
+    return _problem(SYS14, n, n, (0.0, 1.0, 0.0, 1.0), col, bcs, W0, **options)
+
+
 def random_smooth14(nx: int, ny: int, seed: int = SEED, amp: float = 0.2, periodic: bool = True,
                     Kn=None, zsym: bool = False, **options):
     """Generic smooth, fully 3-D non-equilibrium test state on a periodic box: every one of the

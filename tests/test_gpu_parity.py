@@ -349,6 +349,64 @@ def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn):
                 assert np.abs(got[m] - ref[m]).max() <= TOL * scale[m], (ci, cj, m)
 
 
+# ---------------------------------------- the paper's own jet configuration
+@pytest.mark.parametrize("two", [False, True])
+def test_paper_jets_parity(mm, mmo, two):
+    """M = 5 jets of width L/7 into a 1e-5 background, collisionless, Rusanov +
+    van Albada with one shared psi, sigma_lim = 1e-4.
+    This start is the worst-conditioned case in the suite: the fast-wave front sits on the Junk line
+    (sigma just above sigma_lim, closing fluxes ~ 1/sigma^3 sensitive), and an ORACLE run perturbed by
+    1e-15 after every step differs from the unperturbed one by 3e-13 after 2 steps and by 3 % after 3
+    (measured below).  So: element-wise 1e-10 parity over the first 2 steps, the CFL time step of the
+    first steps, and after 100 steps the density field within 10x the oracle's own round-off noise."""
+    prob = wl.paper_jets(64, two=two)
+    dt = 0.5 * scout_dt(mmo, prob, 100, 0.5)
+    Ug, Uo = run_both(mm, mmo, prob, 2, dt=dt, fast=True)
+    assert_parity(Ug, Uo)
+    so = oracle_solver(mmo, prob); sg = mm.Solver.from_problem(prob)
+    for _ in range(2):
+        so.step(1, 0.5); sg.step(1, 0.5)
+        assert sg.info()["last_dt"] == pytest.approx(so.info()["last_dt"], rel=1e-9)
+    # 100 steps: three runs (oracle, perturbed oracle, GPU) compared through the density field
+    so, sp, sg = oracle_solver(mmo, prob), oracle_solver(mmo, prob), mm.Solver.from_problem(prob)
+    rng = np.random.default_rng(1)
+    for _ in range(100):
+        so.step_fixed_dt(1, dt); sp.step_fixed_dt(1, dt)
+        Up = sp.get_state()
+        sp.set_state(Up * (1.0 + 1e-15 * rng.integers(-2, 3, size=Up.shape)))
+    sg.step_fixed_dt(100, dt)
+    Uo, Up, Ug = so.get_state(), sp.get_state(), sg.get_state()
+    noise = np.abs(Up[0] - Uo[0]).mean()
+    assert noise > 1e-9 * np.abs(Uo[0]).mean()              # the ill-conditioning is real
+    assert np.all(np.isfinite(Ug)) and Ug[0].min() > 0
+    assert np.abs(Ug[0] - Uo[0]).mean() <= 10.0 * noise
+    for m in (3, 6, 8, 12):
+        assert np.all(Ug[m] == 0.0)
+    # mass is transported, not created: totals agree to the noise level too
+    assert abs(Ug[0].sum() - Uo[0].sum()) <= 10.0 * max(abs(Up[0].sum() - Uo[0].sum()), 1e-12 * Uo[0].sum())
+
+
+def test_paper_crossing_jets_time_step_drop(mm):
+    """PAPER.md L466-470, Fig 14: the two-jet run needs the same CFL time step as the single-jet run
+    while the jets are independent, and a markedly smaller one once their fast waves interact
+    ("around time step 9000" on the paper's 1200^2 grid, i.e. ~2250 on this 300^2 grid)."""
+    n, chunk, nchunks = 300, 100, 32
+    dts = {}
+    for two in (False, True):
+        s = mm.Solver.from_problem(wl.paper_jets(n, two=two))
+        assert s.fast_path_active
+        h = []
+        for _ in range(nchunks):
+            s.step(chunk, 0.5)
+            h.append(s.info()["last_dt"])
+        U = s.get_state()
+        assert np.all(np.isfinite(U)) and U[0].min() > 0
+        dts[two] = np.array(h)
+    ratio = dts[True] / dts[False]
+    assert np.all(np.abs(ratio[:8] - 1.0) < 0.3)            # steps 100 .. 800: independent jets
+    assert ratio[-3:].max() < 0.5                            # steps 3000 .. 3200: after the interaction
+
+
 # ------------------------------------------------------------------------ error behaviour
 def test_errors_and_failure_flag(mm, mmo):
     with pytest.raises(mm.MMError) as e:
