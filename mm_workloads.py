@@ -23,6 +23,8 @@ TAU_NONE, TAU_CONST, TAU_KN = 0, 1, 2
 BC_TRANSMISSIVE, BC_PERIODIC, BC_DIRICHLET = 0, 1, 2
 LIM_NONE, LIM_MINMOD, LIM_VANALBADA = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
+SRC_EXPLICIT, SRC_POINT_IMPLICIT = 0, 1      # BGK source: forward Euler | point-implicit
+TIME_EULER, TIME_MIDPOINT = 0, 1             # forward Euler | midpoint (2nd-order RK)
 
 SEED = 240115233
 _MASK = (1 << 64) - 1
@@ -58,7 +60,8 @@ def maxwellian(system: int, rho, u=(0.0, 0.0, 0.0), T=1.0) -> np.ndarray:
 
 
 def _problem(system, nx, ny, extent, collision, bcs, W0, **options):
-    opt = dict(sigma_lim=1e-4, ws_scale=1.0, limiter=LIM_MINMOD, shared_limiter=0, flux=FLUX_HLL)
+    opt = dict(sigma_lim=1e-4, ws_scale=1.0, limiter=LIM_MINMOD, shared_limiter=0, flux=FLUX_HLL,
+               source_scheme=SRC_EXPLICIT, time_scheme=TIME_EULER)
     opt.update(options)
     return dict(system=system, nx=nx, ny=ny, extent=extent, collision=collision, bcs=bcs,
                 options=opt, W0=np.ascontiguousarray(W0, dtype=np.float64))

@@ -38,6 +38,8 @@ enum { MMO_TAU_NONE = 0, MMO_TAU_CONST = 1, MMO_TAU_KN = 2 };
 enum { MMO_BC_TRANSMISSIVE = 0, MMO_BC_PERIODIC = 1, MMO_BC_DIRICHLET = 2 };
 enum { MMO_LIM_NONE = 0, MMO_LIM_MINMOD = 1, MMO_LIM_VANALBADA = 2 };
 enum { MMO_FLUX_HLL = 0, MMO_FLUX_RUSANOV = 1 };
+enum { MMO_SRC_EXPLICIT = 0, MMO_SRC_POINT_IMPLICIT = 1 };   /* BGK source: forward Euler | point-implicit (L348) */
+enum { MMO_TIME_EULER = 0, MMO_TIME_MIDPOINT = 1 };          /* L250: forward Euler | midpoint (2nd-order RK) */
 enum { MMO_OK = 0, MMO_EINVAL = -1, MMO_ENONFINITE = -4 };
 
 /* ------------------------------------------------------------------ 5-moment, pointwise */
@@ -128,6 +130,7 @@ typedef struct { int model; double tau, Kn, L_ref, rho_ref; } mmo_collision;
 typedef struct { int type; int nbands; const double *band_lo, *band_hi, *band_W;
                  const double *default_W; } mmo_bc;
 typedef struct { double sigma_lim, ws_scale; int limiter, shared_limiter, flux;
+                 int source_scheme, time_scheme;   /* MMO_SRC_*, MMO_TIME_* (midpoint needs the explicit source) */
                  int nthreads; /* OpenMP threads over rows; <=0: all available */ } mmo_options;
 typedef struct mmo_solver mmo_solver;
 

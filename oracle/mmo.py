@@ -25,6 +25,8 @@ TAU_NONE, TAU_CONST, TAU_KN = 0, 1, 2
 BC_TRANSMISSIVE, BC_PERIODIC, BC_DIRICHLET = 0, 1, 2
 LIM_NONE, LIM_MINMOD, LIM_VANALBADA = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
+SRC_EXPLICIT, SRC_POINT_IMPLICIT = 0, 1      # BGK source: forward Euler | point-implicit
+TIME_EULER, TIME_MIDPOINT = 0, 1             # forward Euler | midpoint (2nd-order RK)
 OK, EINVAL, ENONFINITE = 0, -1, -4
 
 
@@ -58,7 +60,8 @@ class _BC(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("sigma_lim", C.c_double), ("ws_scale", C.c_double), ("limiter", C.c_int),
-                ("shared_limiter", C.c_int), ("flux", C.c_int), ("nthreads", C.c_int)]
+                ("shared_limiter", C.c_int), ("flux", C.c_int), ("source_scheme", C.c_int),
+                ("time_scheme", C.c_int), ("nthreads", C.c_int)]
 
 
 _lib = None
@@ -238,7 +241,7 @@ class Solver:
 
     def __init__(self, system, nx, ny=1, extent=(0.0, 1.0, 0.0, 1.0), collision=None, bcs=None,
                  sigma_lim=1e-4, ws_scale=1.0, limiter=LIM_MINMOD, shared_limiter=0,
-                 flux=FLUX_HLL, nthreads=0):
+                 flux=FLUX_HLL, source_scheme=0, time_scheme=0, nthreads=0):
         L = lib()
         self.nm, self.nx, self.ny = system, nx, ny
         g = _Grid(system, nx, ny, *extent)
@@ -258,7 +261,7 @@ class Solver:
             keep += [lo, hi, bw, dw]
             arr[k] = _BC(b["type"], len(bands), _ptr(lo), _ptr(hi), _ptr(bw),
                          _ptr(dw) if dw is not None else None)
-        o = _Options(sigma_lim, ws_scale, limiter, shared_limiter, flux, nthreads)
+        o = _Options(sigma_lim, ws_scale, limiter, shared_limiter, flux, source_scheme, time_scheme, nthreads)
         h = C.c_void_p()
         rc = L.mmo_create(C.byref(h), C.byref(g), C.byref(c), arr, C.byref(o))
         if rc != OK:

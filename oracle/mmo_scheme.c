@@ -86,6 +86,7 @@ struct mmo_solver {
     int nm, ndim, sx, sy;     /* moments per cell, space dimensions, padded sizes */
     double dx, dy;
     double *U, *W, *Un;       /* [sy][sx][nm] with ghosts */
+    double *U0;               /* midpoint scheme: U^n kept while the half step is in U */
     double *Fx, *Fy;          /* [ny][nx+1][nm], [ny+1][nx][nm] */
     double t, last_dt;
     long long steps;
@@ -129,6 +130,8 @@ int mmo_create(mmo_solver **out, const mmo_grid *g, const mmo_collision *c,
     if (g->system == MMO_SYS5_1D && g->ny != 1) return MMO_EINVAL;
     if (g->system == MMO_SYS14_2D && !(g->y1 > g->y0)) return MMO_EINVAL;
     if (!(o->sigma_lim > 0.0) || !(o->ws_scale > 0.0)) return MMO_EINVAL;
+    if (o->source_scheme < 0 || o->source_scheme > 1 || o->time_scheme < 0 || o->time_scheme > 1) return MMO_EINVAL;
+    if (o->time_scheme == MMO_TIME_MIDPOINT && o->source_scheme != MMO_SRC_EXPLICIT) return MMO_EINVAL;
     mmo_solver *s = (mmo_solver *)calloc(1, sizeof *s);
     if (!s) return MMO_EINVAL;
     s->g = *g; s->col = *c; s->opt = *o;
@@ -165,9 +168,10 @@ int mmo_create(mmo_solver **out, const mmo_grid *g, const mmo_collision *c,
     s->U = (double *)calloc(ncell * s->nm, sizeof(double));
     s->W = (double *)calloc(ncell * s->nm, sizeof(double));
     s->Un = (double *)calloc(ncell * s->nm, sizeof(double));
+    s->U0 = (double *)calloc(ncell * s->nm, sizeof(double));
     s->Fx = (double *)calloc((size_t)g->ny * (g->nx + 1) * s->nm, sizeof(double));
     s->Fy = (double *)calloc((size_t)(g->ny + 1) * g->nx * s->nm, sizeof(double));
-    if (!s->U || !s->W || !s->Un || !s->Fx || !s->Fy) { mmo_destroy(s); return MMO_EINVAL; }
+    if (!s->U || !s->W || !s->Un || !s->U0 || !s->Fx || !s->Fy) { mmo_destroy(s); return MMO_EINVAL; }
     int nt = o->nthreads;
 #ifdef _OPENMP
     if (nt <= 0) nt = omp_get_max_threads();
@@ -183,7 +187,7 @@ void mmo_destroy(mmo_solver *s)
 {
     if (!s) return;
     for (int b = 0; b < 4; ++b) free(s->bc_store[b]);
-    free(s->U); free(s->W); free(s->Un); free(s->Fx); free(s->Fy);
+    free(s->U); free(s->W); free(s->Un); free(s->U0); free(s->Fx); free(s->Fy);
     free(s);
 }
 
@@ -401,31 +405,65 @@ static void all_fluxes(mmo_solver *s)
     }
 }
 
-/* ---- step 6: U^{n+1} = U^n - dt/dx (Fx_{i+1/2} - Fx_{i-1/2}) - dt/dy (Fy_{j+1/2} - Fy_{j-1/2})
- *                        + dt C(U^n), tau from the cell's own W^n (L250; Eqs 12, 17-18). */
-static void update(mmo_solver *s, double dt)
+/* Moments of the Maxwellian with the density, velocity and hydrostatic pressure of W (L73, L127):
+ * the equilibrium the BGK operator relaxes to (Eqs 17-18; Eq 12d-e). */
+static void equilibrium_of(const mmo_solver *s, const double *W, double *Ueq)
+{
+    double Weq[14];
+    double P = hydrostatic(s, W);
+    if (s->nm == 5) {
+        Weq[0] = W[0]; Weq[1] = W[1]; Weq[2] = P; Weq[3] = 0.0; Weq[4] = 3.0 * P * P / W[0];
+    } else {
+        for (int m = 0; m < 14; ++m) Weq[m] = 0.0;
+        Weq[0] = W[0]; Weq[1] = W[1]; Weq[2] = W[2]; Weq[3] = W[3];
+        Weq[4] = P; Weq[7] = P; Weq[9] = P;
+        Weq[13] = 15.0 * P * P / W[0];
+    }
+    p2c(s, Weq, Ueq);
+}
+
+/* ---- step 6: U^{new} = B - dt/dx (Fx_{i+1/2} - Fx_{i-1/2}) - dt/dy (Fy_{j+1/2} - Fy_{j-1/2}) + source,
+ * with the fluxes and primitives W of the state currently in s->U, and B = `base` (U^n itself for
+ * forward Euler; U^n while s->U holds the half step of the midpoint scheme, L250).
+ * Source, explicit:        + dt C(W), tau from the cell's own W (L250; Eqs 12, 17-18).
+ * Source, point-implicit (L348): with U* the flux-updated state, the BGK relaxation is integrated by
+ *   backward Euler, U^{new} = (U* + (dt/tau) U_eq) / (1 + dt/tau); U_eq and tau depend only on rho, u
+ *   and the hydrostatic pressure, which the source does not change, so they are those of U*. */
+static void update(mmo_solver *s, double dt, const double *base)
 {
     int nx = s->g.nx, ny = s->g.ny, nm = s->nm;
 #pragma omp parallel for num_threads(s->nthreads) schedule(static)
     for (int j = 0; j < ny; ++j)
         for (int i = 0; i < nx; ++i) {
-            const double *U = s->U + cidx(s, i, j), *W = s->W + cidx(s, i, j);
+            const double *U = base + cidx(s, i, j), *W = s->W + cidx(s, i, j);
             double *Un = s->Un + cidx(s, i, j);
             const double *Fw = s->Fx + ((size_t)j * (nx + 1) + i) * nm, *Fe = Fw + nm;
-            double C[14];
-            double tau = mmo_tau(s->col.model, s->col.tau, s->col.Kn, s->col.L_ref,
-                                 s->col.rho_ref, W[0], hydrostatic(s, W));
-            if (s->col.model == MMO_TAU_NONE) for (int m = 0; m < nm; ++m) C[m] = 0.0;
-            else if (nm == 5) mmo_source5(W, tau, C);
-            else mmo_source14(W, tau, C);
+            double v[14];
             for (int m = 0; m < nm; ++m) {
-                double v = U[m] - dt / s->dx * (Fe[m] - Fw[m]);
+                v[m] = U[m] - dt / s->dx * (Fe[m] - Fw[m]);
                 if (s->ndim == 2) {
                     const double *Fs = s->Fy + ((size_t)j * nx + i) * nm;
                     const double *Fn = s->Fy + ((size_t)(j + 1) * nx + i) * nm;
-                    v -= dt / s->dy * (Fn[m] - Fs[m]);
+                    v[m] -= dt / s->dy * (Fn[m] - Fs[m]);
                 }
-                Un[m] = v + dt * C[m];
+            }
+            if (s->col.model == MMO_TAU_NONE) {
+                for (int m = 0; m < nm; ++m) Un[m] = v[m];
+            } else if (s->opt.source_scheme == MMO_SRC_POINT_IMPLICIT) {
+                double Ws[14], Ueq[14];
+                c2p(s, v, Ws);
+                double tau = mmo_tau(s->col.model, s->col.tau, s->col.Kn, s->col.L_ref,
+                                     s->col.rho_ref, Ws[0], hydrostatic(s, Ws));
+                equilibrium_of(s, Ws, Ueq);
+                double x = dt / tau;
+                for (int m = 0; m < nm; ++m) Un[m] = (v[m] + x * Ueq[m]) / (1.0 + x);
+            } else {
+                double C[14];
+                double tau = mmo_tau(s->col.model, s->col.tau, s->col.Kn, s->col.L_ref,
+                                     s->col.rho_ref, W[0], hydrostatic(s, W));
+                if (nm == 5) mmo_source5(W, tau, C);
+                else mmo_source14(W, tau, C);
+                for (int m = 0; m < nm; ++m) Un[m] = v[m] + dt * C[m];
             }
         }
     double *tmp = s->U; s->U = s->Un; s->Un = tmp;
@@ -444,8 +482,20 @@ static int one_step(mmo_solver *s, double dt_fixed, double cfl, double t_end)
     }
     int last = t_end > s->t && s->t + dt >= t_end;               /* land on t_end */
     if (last) dt = t_end - s->t;
-    all_fluxes(s);
-    update(s, dt);
+    if (s->opt.time_scheme == MMO_TIME_MIDPOINT) {
+        /* L250 "midpoint Euler (2nd order Runge-Kutta)": U' = U^n + dt/2 L(U^n); U^{n+1} = U^n + dt L(U') */
+        size_t nbytes = (size_t)s->sx * s->sy * s->nm * sizeof(double);
+        memcpy(s->U0, s->U, nbytes);
+        all_fluxes(s);
+        update(s, 0.5 * dt, s->U0);
+        fill_ghosts(s);
+        all_cons2prim(s);
+        all_fluxes(s);
+        update(s, dt, s->U0);
+    } else {
+        all_fluxes(s);
+        update(s, dt, s->U);
+    }
     if (last) s->t = t_end; else s->t += dt;
     s->last_dt = dt;
     s->steps += 1;

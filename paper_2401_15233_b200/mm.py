@@ -18,6 +18,8 @@ TAU_NONE, TAU_CONST, TAU_KN = 0, 1, 2
 BC_TRANSMISSIVE, BC_PERIODIC, BC_DIRICHLET = 0, 1, 2
 LIM_NONE, LIM_MINMOD, LIM_VANALBADA = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
+SRC_EXPLICIT, SRC_POINT_IMPLICIT = 0, 1      # BGK source: forward Euler | point-implicit
+TIME_EULER, TIME_MIDPOINT = 0, 1             # forward Euler | midpoint (2nd-order RK)
 OK, EINVAL, EWORKSPACE, ECUDA, ENONFINITE = 0, -1, -2, -3, -4
 MAX_BANDS = 8
 
