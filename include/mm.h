@@ -47,6 +47,8 @@ enum { MM_TAU_NONE = 0, MM_TAU_CONST = 1, MM_TAU_KN = 2 };
 enum { MM_BC_TRANSMISSIVE = 0, MM_BC_PERIODIC = 1, MM_BC_DIRICHLET = 2 };
 enum { MM_LIM_NONE = 0, MM_LIM_MINMOD = 1, MM_LIM_VANALBADA = 2 };
 enum { MM_FLUX_HLL = 0, MM_FLUX_RUSANOV = 1 };
+enum { MM_SRC_EXPLICIT = 0, MM_SRC_POINT_IMPLICIT = 1 };
+enum { MM_TIME_EULER = 0, MM_TIME_MIDPOINT = 1 };
 #define MM_MAX_BANDS 8
 
 typedef struct mm_solver mm_solver;   /* opaque, host object; freed by mm_destroy */
@@ -77,6 +79,12 @@ typedef struct {
     int limiter;          /* MM_LIM_MINMOD | MM_LIM_VANALBADA (L262) | MM_LIM_NONE (1st order) */
     int shared_limiter;   /* 1: the most stringent limiter value for all primitives (L266) */
     int flux;             /* MM_FLUX_HLL | MM_FLUX_RUSANOV (L258) */
+    int source_scheme;    /* MM_SRC_EXPLICIT: + dt C(W^n), forward Euler (L250) | MM_SRC_POINT_IMPLICIT (L348):
+                           * with U* the flux-updated state, U^{n+1} = (U* + (dt/tau) U_eq)/(1 + dt/tau);
+                           * U_eq, tau from rho, u, hydrostatic P of U* (collision invariants) */
+    int time_scheme;      /* MM_TIME_EULER (L250, L434) | MM_TIME_MIDPOINT (L250, 2nd-order Runge-Kutta):
+                           * U' = U^n + dt/2 L(U^n), U^{n+1} = U^n + dt L(U'), dt from the CFL rate of U^n;
+                           * two kernel passes per step; requires MM_SRC_EXPLICIT */
     void *stream;         /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
 } mm_options;
 

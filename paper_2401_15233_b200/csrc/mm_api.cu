@@ -97,6 +97,7 @@ struct mm_solver {
     int has_state;
     long long launches;
     int nstrips, nchunks[2];   // 14-moment work decomposition (mm_strip14.cuh): [general, z-symmetric]
+    int time_scheme;        // MM_TIME_EULER | MM_TIME_MIDPOINT
     int zsym;               // state and boundary data have no z-odd moment: fast path applies
     int allow_fast;         // mm_set_fast_path
     int sms;
@@ -127,39 +128,65 @@ int launch_ghost(mm_solver* s, const StepCtl& sc, int finalize)
     return MM_OK;
 }
 
-int launch_step(mm_solver* s, const StepCtl& sc)
+// one pass of the fused step kernel: U[out] = B - dt_scale dt div F(U[in]) + source
+int launch_pass(mm_solver* s, int in, int out, const double* base, double dt_scale, int do_rate)
+{
+    if (s->L.nm == 5) {
+        const int nb = (s->p.nx + kNT5 - 1) / kNT5;
+        k_step5<kNT5><<<nb, kNT5, 0, s->stream>>>(s->p, s->U[in], s->U[out], s->ctrl, s->slot ^ 1, base, dt_scale, do_rate);
+        MM_LAUNCHED(s, "k_step5");
+    } else {
+        const int fast = s->zsym && s->allow_fast;
+        const int items = s->nstrips * s->nchunks[fast];
+        const int nb = (items + kStripWPB - 1) / kStripWPB;
+        const bool ext = base != nullptr || dt_scale != 1.0 || !do_rate || s->p.source_scheme != 0;
+#define MM_LAUNCH_STRIP(ZSV, MINB, SMEM, NCH, EXTV)                                                   \
+    k_step14_strip<ZSV, MINB, EXTV><<<nb, 32 * kStripWPB, SMEM, s->stream>>>(                         \
+        s->p, s->U[in], s->U[out], s->ctrl, s->slot ^ 1, s->nstrips, NCH, base, dt_scale, do_rate)
+        if (fast) { if (ext) MM_LAUNCH_STRIP(true, kMinBlocksZS, kSmemZS, s->nchunks[1], true);
+                    else MM_LAUNCH_STRIP(true, kMinBlocksZS, kSmemZS, s->nchunks[1], false); }
+        else { if (ext) MM_LAUNCH_STRIP(false, kMinBlocksGen, kSmemGen, s->nchunks[0], true);
+               else MM_LAUNCH_STRIP(false, kMinBlocksGen, kSmemGen, s->nchunks[0], false); }
+#undef MM_LAUNCH_STRIP
+        MM_LAUNCHED(s, "k_step14_strip");
+    }
+    return MM_OK;
+}
+
+template <int NM>
+int launch_step_nm(mm_solver* s, const StepCtl& sc, cudaEvent_t e0, cudaEvent_t e1)
 {
     int rc;
+    if ((rc = launch_ghost<NM>(s, sc, 1))) return rc;            // ghosts of U^n, dt from its CFL rate
+    if (e0) MM_CUDA(cudaEventRecord(e0, s->stream));
+    const int a = s->cur, b = s->cur ^ 1;
+    if (s->time_scheme == MM_TIME_MIDPOINT) {
+        // U' = U^n + dt/2 L(U^n) -> b;  ghosts of U';  U^{n+1} = U^n + dt L(U') -> a, in place
+        if ((rc = launch_pass(s, a, b, nullptr, 0.5, 0))) return rc;
+        s->cur = b;
+        StepCtl none = {0, 0.0, -1.0};
+        rc = launch_ghost<NM>(s, none, 0);
+        s->cur = a;
+        if (rc) return rc;
+        if ((rc = launch_pass(s, b, a, s->U[a], 1.0, 1))) return rc;
+    } else {
+        if ((rc = launch_pass(s, a, b, nullptr, 1.0, 1))) return rc;
+        s->cur = b;
+    }
+    if (e1) MM_CUDA(cudaEventRecord(e1, s->stream));
+    s->slot ^= 1;
+    return MM_OK;
+}
+
+int launch_step(mm_solver* s, const StepCtl& sc)
+{
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (s->profiling) {
         MM_CUDA(cudaEventCreate(&e0));
         MM_CUDA(cudaEventCreate(&e1));
         s->ev.push_back(e0); s->ev.push_back(e1);
     }
-    if (s->L.nm == 5) {
-        if ((rc = launch_ghost<5>(s, sc, 1))) return rc;
-        const int nb = (s->p.nx + kNT5 - 1) / kNT5;
-        if (e0) MM_CUDA(cudaEventRecord(e0, s->stream));
-        k_step5<kNT5><<<nb, kNT5, 0, s->stream>>>(s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1);
-        MM_LAUNCHED(s, "k_step5");
-    } else {
-        if ((rc = launch_ghost<14>(s, sc, 1))) return rc;
-        const int fast = s->zsym && s->allow_fast;
-        const int items = s->nstrips * s->nchunks[fast];
-        const int nb = (items + kStripWPB - 1) / kStripWPB;
-        if (e0) MM_CUDA(cudaEventRecord(e0, s->stream));
-        if (fast)
-            k_step14_strip<true, kMinBlocksZS><<<nb, 32 * kStripWPB, kSmemZS, s->stream>>>(
-                s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks[1]);
-        else
-            k_step14_strip<false, kMinBlocksGen><<<nb, 32 * kStripWPB, kSmemGen, s->stream>>>(
-                s->p, s->U[s->cur], s->U[s->cur ^ 1], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks[0]);
-        MM_LAUNCHED(s, "k_step14_strip");
-    }
-    if (e1) MM_CUDA(cudaEventRecord(e1, s->stream));
-    s->cur ^= 1;
-    s->slot ^= 1;
-    return MM_OK;
+    return s->L.nm == 5 ? launch_step_nm<5>(s, sc, e0, e1) : launch_step_nm<14>(s, sc, e0, e1);
 }
 
 int read_ctrl(mm_solver* s, Ctrl* h)
@@ -238,6 +265,8 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
     if (!make_layout(grid, &L)) return MM_EINVAL;
     if (!(opt->sigma_lim > 0.0) || !(opt->ws_scale > 0.0)) return MM_EINVAL;
     if (opt->limiter < 0 || opt->limiter > 2 || opt->flux < 0 || opt->flux > 1) return MM_EINVAL;
+    if (opt->source_scheme < 0 || opt->source_scheme > 1 || opt->time_scheme < 0 || opt->time_scheme > 1) return MM_EINVAL;
+    if (opt->time_scheme == MM_TIME_MIDPOINT && opt->source_scheme != MM_SRC_EXPLICIT) return MM_EINVAL;
     if (col->model < 0 || col->model > 2) return MM_EINVAL;
     if (col->model == MM_TAU_CONST && !(col->tau > 0.0)) return MM_EINVAL;
     if (col->model == MM_TAU_KN && !(col->Kn > 0.0 && col->L_ref > 0.0 && col->rho_ref > 0.0)) return MM_EINVAL;
@@ -275,6 +304,7 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
     p.inv_tau_const = col->model == MM_TAU_CONST ? 1.0 / col->tau : 0.0;
     p.tau_model = col->model; p.limiter = opt->limiter;
     p.shared_limiter = opt->shared_limiter ? 1 : 0; p.flux = opt->flux;
+    p.source_scheme = opt->source_scheme; s->time_scheme = opt->time_scheme;
     p.nx = grid->nx; p.ny = grid->ny; p.pitch = L.pitch; p.rows = L.rows;
     p.ab = (const double*)(s->ws + L.off_tab);
 
@@ -313,9 +343,13 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
     if (nm == 14) {
         k_ab_table<<<AbTable::kIntervals, 2, 0, s->stream>>>((double*)(s->ws + L.off_tab));
         s->launches++;
-        e = cudaFuncSetAttribute(k_step14_strip<false, kMinBlocksGen>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
+        e = cudaFuncSetAttribute(k_step14_strip<false, kMinBlocksGen, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(k_step14_strip<true, kMinBlocksZS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
+            e = cudaFuncSetAttribute(k_step14_strip<false, kMinBlocksGen, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_step14_strip<true, kMinBlocksZS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_step14_strip<true, kMinBlocksZS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
         if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaFuncSetAttribute(k_step14_strip)"); }
         int dev = 0, sms = 148;
         cudaGetDevice(&dev);

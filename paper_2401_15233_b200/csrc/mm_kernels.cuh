@@ -312,7 +312,8 @@ __device__ __forceinline__ void interface_flux5(const Params& p, const double* _
 // 5-moment 1-D step: one block = NT consecutive cells, same four stages.
 template <int NT>
 __global__ void __launch_bounds__(NT)
-k_step5(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl, int slot_next)
+k_step5(Params p, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl, int slot_next,
+        const double* Ubase, double dt_scale, int do_rate)
 {
     constexpr int NM = 5, PW = NT + 4, PF = NT + 1;
     __shared__ double Ws[NM * PW];
@@ -320,7 +321,7 @@ k_step5(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctr
     const int tid = threadIdx.x, gx0 = blockIdx.x * NT;
     const size_t plane = (size_t)p.rows * p.pitch;
     const size_t row = (size_t)2 * p.pitch;
-    const double dt = ctrl->dt;
+    const double dt = ctrl->dt * dt_scale;          // see k_step14_strip for Ubase / dt_scale / do_rate
     const bool cell_ok = gx0 + tid < p.nx;
     const size_t cidx = row + gx0 + tid + 2;
     if (ctrl->skip) {
@@ -354,15 +355,24 @@ k_step5(Params p, const double* __restrict__ Uin, double* __restrict__ Uout, Ctr
         double Un[NM], W[NM];
 #pragma unroll
         for (int m = 0; m < NM; ++m) {
-            Un[m] = Uin[m * plane + cidx] - dtdx * (Fx[m * PF + tid + 1] - Fx[m * PF + tid]);
+            Un[m] = (Ubase ? Ubase : Uin)[m * plane + cidx] - dtdx * (Fx[m * PF + tid + 1] - Fx[m * PF + tid]);
             W[m] = Ws[m * PW + tid + 2];
         }
-        if (p.tau_model != 0) add_source5(W, dt * inv_tau(p, W[0], W[2]), Un);
+        if (p.tau_model != 0) {
+            if (p.source_scheme == 1) {                  // point-implicit (L348): relax U* itself
+                double Wst[NM];
+                cons2prim5(Un, Wst);
+                const double x = dt * inv_tau(p, Wst[0], Wst[2]);
+                add_source5(Wst, x / (1.0 + x), Un);
+            } else {
+                add_source5(W, dt * inv_tau(p, W[0], W[2]), Un);
+            }
+        }
 #pragma unroll
         for (int m = 0; m < NM; ++m) Uout[m * plane + cidx] = Un[m];
-        cell_rate<NM>(p, Un, rate, speed, bad);
+        if (do_rate) cell_rate<NM>(p, Un, rate, speed, bad);
     }
-    block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
+    if (do_rate) block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
 }
 
 // Register-resident DFMA loop: 16 independent chains per thread, 2 flop per FMA.

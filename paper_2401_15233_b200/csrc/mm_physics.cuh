@@ -113,6 +113,7 @@ struct Params {               // per-solver constants, passed by value to the ke
     double inv_tau_coef;      // MM_TAU_KN: 1/tau = inv_tau_coef * rho * sqrt(8 P /(pi rho))
     double inv_tau_const;     // MM_TAU_CONST: 1/tau
     int tau_model, limiter, shared_limiter, flux;
+    int source_scheme;        // 0 explicit, 1 point-implicit (L348)
     int nx, ny, pitch, rows;  // padded array: rows x pitch doubles per moment, interior at (+2,+2)
     const double* ab;         // table of the functions a(P*), b(P*) of Eq 29c-d (AbTable below)
 };

@@ -61,15 +61,21 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // Work decomposition: item = (strip, chunk); chunk c covers rows [c ny / nchunks, (c+1) ny / nchunks).
-template <bool ZS, int MINB>
+// EXT = false is the plain forward-Euler step with the explicit source (Ubase = nullptr,
+// dt_scale = 1, do_rate = 1, source_scheme = 0 folded at compile time); EXT = true takes them at
+// run time (midpoint passes, point-implicit source).
+template <bool ZS, int MINB, bool EXT>
 #ifdef MM_MAXNREG
 __global__ void __maxnreg__(MM_MAXNREG)
 #else
 __global__ void __launch_bounds__(32 * kStripWPB, MINB)
 #endif
-k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restrict__ Uout, Ctrl* ctrl,
-               int slot_next, int nstrips, int nchunks)
+k_step14_strip(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl,
+               int slot_next, int nstrips, int nchunks, const double* Ubase_, double dt_scale_, int do_rate_)
 {
+    const double* Ubase = EXT ? Ubase_ : nullptr;
+    const double dt_scale = EXT ? dt_scale_ : 1.0;
+    const int do_rate = EXT ? do_rate_ : 1;
     using Z = typename std::conditional<ZS, zero_t, double>::type;
     using M = Mom<ZS>;
     constexpr int NM = 14, NV = M::NV, RS = NV * kRW;          // RS: doubles per staged row
@@ -107,7 +113,10 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restri
                     Uout[m * plane + (size_t)(r + 2) * p.pitch + ccol] = Uin[m * plane + (size_t)(r + 2) * p.pitch + ccol];
         return;
     }
-    const double dt = ctrl->dt;
+    // U_out = B - dt div F(U_in) + source:  B = U_in for forward Euler and for the half step of the
+    // midpoint scheme (dt_scale = 1/2, no CFL reduction); B = Ubase = U^n for its full step, which
+    // may be written in place (Uout == Ubase: a cell's B is read by the lane that later writes it).
+    const double dt = ctrl->dt * dt_scale;
     const double dtdx = dt / p.dx, dtdy = dt / p.dy;
 
     auto load_row = [&](int r, int cslot) {          // interior row r in [-2, ny+1] -> cons[cslot]
@@ -246,22 +255,39 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restri
                             Un[M::full(k)] = __dsub_rn(acc[k * 32 + lane], __dmul_rn(dtdy, G[k]));
                             W[M::full(k)] = w[k * kRW];
                         }
-                        if (p.tau_model != 0)
-                            add_source14<Z>(W, dt * inv_tau(p, W[0], (W[4] + W[7] + W[9]) * (1.0 / 3.0)), Un);
+                        if (p.tau_model != 0) {
+                            if (EXT && p.source_scheme == 1) {   // point-implicit (L348): relax U* itself
+                                double Ws[NM];
+                                cons2prim14<Z>(Un, Ws);
+                                const double x = dt * inv_tau(p, Ws[0], (Ws[4] + Ws[7] + Ws[9]) * (1.0 / 3.0));
+                                add_source14<Z>(Ws, x * rcp(1.0 + x), Un);
+                            } else {
+                                add_source14<Z>(W, dt * inv_tau(p, W[0], (W[4] + W[7] + W[9]) * (1.0 / 3.0)), Un);
+                            }
+                        }
                         double* out = Uout + (size_t)(r + 1) * p.pitch + ccol;
 #pragma unroll
                         for (int m = 0; m < NM; ++m) {
                             if (ZS && z_odd(m)) out[m * plane] = 0.0;
                             else out[m * plane] = Un[m];
                         }
-                        double rr, ss;
-                        cell_rate<NM, Z>(p, Un, rr, ss, bad);
-                        rate = dmax(rate, rr); speed = dmax(speed, ss);
+                        if (do_rate) {
+                            double rr, ss;
+                            cell_rate<NM, Z>(p, Un, rr, ss, bad);
+                            rate = dmax(rate, rr); speed = dmax(speed, ss);
+                        }
                     }
                     if (r < y1) {
+                        if (Ubase) {
+                            const double* ub = Ubase + (size_t)(r + 2) * p.pitch + ccol;
 #pragma unroll
-                        for (int k = 0; k < NV; ++k)
-                            acc[k * 32 + lane] = __dadd_rn(cons[cs * RS + k * kRW + lane + 2], __dmul_rn(dtdy, G[k]));
+                            for (int k = 0; k < NV; ++k)
+                                acc[k * 32 + lane] = __dadd_rn(ub[M::full(k) * plane], __dmul_rn(dtdy, G[k]));
+                        } else {
+#pragma unroll
+                            for (int k = 0; k < NV; ++k)
+                                acc[k * 32 + lane] = __dadd_rn(cons[cs * RS + k * kRW + lane + 2], __dmul_rn(dtdy, G[k]));
+                        }
                     }
                 }
             } else {
@@ -286,7 +312,7 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* __restri
         speed = fmax(speed, __shfl_xor_sync(0xffffffffu, speed, o));
         bad |= __shfl_xor_sync(0xffffffffu, bad, o);
     }
-    if (lane == 0) {
+    if (lane == 0 && do_rate) {
         atomic_max_pos(&ctrl->rate_bits[slot_next], rate);
         atomic_max_pos(&ctrl->speed_bits[slot_next], speed);
         if (bad) atomicOr(&ctrl->bad[slot_next], 1);

@@ -49,7 +49,8 @@ class mm_bc(C.Structure):
 
 class mm_options(C.Structure):
     _fields_ = [("sigma_lim", C.c_double), ("ws_scale", C.c_double), ("limiter", C.c_int),
-                ("shared_limiter", C.c_int), ("flux", C.c_int), ("stream", C.c_void_p)]
+                ("shared_limiter", C.c_int), ("flux", C.c_int), ("source_scheme", C.c_int),
+                ("time_scheme", C.c_int), ("stream", C.c_void_p)]
 
 
 class MMError(RuntimeError):
@@ -142,7 +143,8 @@ class Solver:
     def __init__(self, system: int, nx: int, ny: int = 1, extent=(0.0, 1.0, 0.0, 1.0),
                  collision: Optional[dict] = None, bcs: Optional[Sequence[dict]] = None,
                  sigma_lim: float = 1e-4, ws_scale: float = 1.0, limiter: int = LIM_MINMOD,
-                 shared_limiter: int = 0, flux: int = FLUX_HLL, device: str = "cuda:0", stream=None):
+                 shared_limiter: int = 0, flux: int = FLUX_HLL, source_scheme: int = SRC_EXPLICIT,
+                 time_scheme: int = TIME_EULER, device: str = "cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise MMError(ECUDA, "no CUDA device: the moment-method library has no CPU path")
@@ -174,7 +176,7 @@ class Solver:
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = self.workspace.data_ptr()
             self._ws_ptr = (base + 255) // 256 * 256
-            o = mm_options(sigma_lim, ws_scale, limiter, shared_limiter, flux,
+            o = mm_options(sigma_lim, ws_scale, limiter, shared_limiter, flux, source_scheme, time_scheme,
                            C.c_void_p(self._stream.cuda_stream))
             h = C.c_void_p()
             _check(L.mm_create(C.byref(h), C.byref(g), C.byref(c), arr, C.byref(o),

@@ -38,7 +38,7 @@ def test_binding_structs_match_header(mm):
     assert [f[0] for f in mm.mm_grid._fields_] == ["system", "nx", "ny", "x0", "x1", "y0", "y1"]
     assert [f[0] for f in mm.mm_collision._fields_] == ["model", "tau", "Kn", "L_ref", "rho_ref"]
     assert [f[0] for f in mm.mm_bc._fields_] == ["type", "nbands", "band_lo", "band_hi", "band_W", "default_W"]
-    assert [f[0] for f in mm.mm_options._fields_] == ["sigma_lim", "ws_scale", "limiter", "shared_limiter", "flux", "stream"]
+    assert [f[0] for f in mm.mm_options._fields_] == ["sigma_lim", "ws_scale", "limiter", "shared_limiter", "flux", "source_scheme", "time_scheme", "stream"]
     for name, val in [("MM_SYS5_1D", 5), ("MM_SYS14_2D", 14), ("MM_MAX_BANDS", 8)]:
         assert re.search(rf"{name}\s*=?\s*{val}\b", text)
 
@@ -57,7 +57,7 @@ def test_workspace_bytes_and_argument_checks(mm):
     # NULL / bad arguments are rejected before any CUDA call
     g = mm.mm_grid(14, 8, 8, 0, 1, 0, 1)
     c = mm.mm_collision(0, 0, 0, 1, 1)
-    o = mm.mm_options(1e-4, 1.0, 1, 0, 0, None)
+    o = mm.mm_options(1e-4, 1.0, 1, 0, 0, 0, 0, None)
     b = (mm.mm_bc * 4)()
     h = C.c_void_p()
     assert lib.mm_create(C.byref(h), C.byref(g), C.byref(c), b, C.byref(o), None, 0) == mm.EWORKSPACE
@@ -78,7 +78,7 @@ def test_no_cpu_fallback(mm):
     lib = mm.lib()
     g = mm.mm_grid(5, 8, 1, 0, 1, 0, 1)
     c = mm.mm_collision(0, 0, 0, 1, 1)
-    o = mm.mm_options(1e-4, 1.0, 1, 0, 0, None)
+    o = mm.mm_options(1e-4, 1.0, 1, 0, 0, 0, 0, None)
     b = (mm.mm_bc * 4)()
     h = C.c_void_p()
     n = lib.mm_workspace_bytes(C.byref(g))

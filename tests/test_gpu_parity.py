@@ -349,6 +349,47 @@ def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn):
                 assert np.abs(got[m] - ref[m]).max() <= TOL * scale[m], (ci, cj, m)
 
 
+# ----------------- midpoint time marching (L250), point-implicit source (L348)
+@pytest.mark.parametrize("opts", [dict(source_scheme=wl.SRC_POINT_IMPLICIT), dict(time_scheme=wl.TIME_MIDPOINT)])
+@pytest.mark.parametrize("case", ["smooth14", "smooth14_zsym", "smooth5", "jets", "sod14"])
+def test_time_and_source_schemes(mm, mmo, opts, case):
+    if case == "smooth14":
+        prob, n, cfl = wl.random_smooth14(70, 37, Kn=0.05, **opts), 30, 0.4
+    elif case == "smooth14_zsym":
+        prob, n, cfl = wl.random_smooth14(70, 37, Kn=0.05, zsym=True, flux=wl.FLUX_RUSANOV, **opts), 30, 0.4
+    elif case == "smooth5":
+        prob, n, cfl = wl.random_smooth5(333, Kn=0.05, **opts), 100, 0.5
+    elif case == "jets":
+        prob, n, cfl = wl.crossed_jets(96, Kn=1.0, **opts), 100, 0.4
+    else:
+        prob, n, cfl = wl.sod14(1024, 4, Kn=1e-3, **opts), 100, 0.5
+    Ug, Uo = run_both(mm, mmo, prob, n, cfl=cfl)
+    assert_parity(Ug, Uo)
+    # CFL stepping: same dt sequence (the midpoint scheme takes dt from the CFL rate of U^n)
+    so = oracle_solver(mmo, prob); sg = mm.Solver.from_problem(prob)
+    so.step(10, cfl); sg.step(10, cfl)
+    assert sg.info()["t"] == pytest.approx(so.info()["t"], rel=1e-10)
+    assert sg.info()["steps"] == 10
+
+
+def test_point_implicit_sod5_small_knudsen(mm, mmo):
+    """dt ~ 30 tau (Kn = 1e-5, CFL 0.5): the point-implicit source runs the whole tube to t = 0.2 and
+    matches the oracle; both reproduce the Euler (gamma = 3) limit (oracle pin in test_oracle_scheme)."""
+    prob = wl.sod5(400, Kn=1e-5, source_scheme=wl.SRC_POINT_IMPLICIT)
+    so = oracle_solver(mmo, prob); sg = mm.Solver.from_problem(prob)
+    so.advance_to(0.2, 0.5); sg.advance_to(0.2, 0.5)
+    assert sg.info()["steps"] == so.info()["steps"]
+    assert_parity(sg.get_state(), so.get_state(), 1e-9)
+
+
+def test_scheme_option_errors(mm):
+    with pytest.raises(mm.MMError) as e:
+        mm.Solver(14, 8, 8, time_scheme=wl.TIME_MIDPOINT, source_scheme=wl.SRC_POINT_IMPLICIT)
+    assert e.value.status == mm.EINVAL
+    with pytest.raises(mm.MMError):
+        mm.Solver(14, 8, 8, time_scheme=2)
+
+
 # ---------------------------------------- SURVEY 8(f) item 1: the paper's own jet configuration
 @pytest.mark.parametrize("two", [False, True])
 def test_paper_jets_parity(mm, mmo, two):
