@@ -35,17 +35,17 @@ UNIT = "cell-updates/s"
 CFL = 0.4
 
 
-def flops_per_cell_update(shared_limiter: bool, zsym: bool):
+def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14):
     """Algorithmic FP64 operations per cell update (each + - * / sqrt exp log = 1).
     -> (count of the formulation the CUDA path runs, count of the oracle's naive restatement).
     The roofline line uses the FIRST (smaller) number: flops the kernel does not execute are not
     credited to it.  Both are produced by committed counting builds, not typed in."""
     from paper_2401_15233_b200 import build_ext
-    k = build_ext.read_opcount()["kernel_flops_per_cell_update_14_" + ("zsym_" if zsym else "")
+    k = build_ext.read_opcount()[f"kernel_flops_per_cell_update_{system}_" + ("zsym_" if zsym and system == 14 else "")
                                  + ("shared_limiter" if shared_limiter else "per_variable_limiter")]
     o = None
     for line in (ROOT / "tests" / "golden" / "oracle_opcount.txt").read_text().splitlines():
-        if line.startswith("flops_per_cell_update_14 "):
+        if line.startswith(f"flops_per_cell_update_{system} "):
             o = float(line.split()[1])
     return float(k), o
 
@@ -129,6 +129,12 @@ WORKLOADS = {
     "paper-single": (lambda n, kn: wl.paper_jets(n, two=False), 0.5,
                      "the paper's collisionless M=5 single jet {n}x{n} (PAPER.md L430-444), van Albada (shared "
                      "psi) + Rusanov, CFL 0.5; SURVEY 8(f) item 1, not the BASELINE metric's workload"),
+    "sod5": (lambda n, kn: wl.sod5(n, Kn=kn), 0.5,
+             "1-D 5-moment Sod tube, {n} cells, Kn={kn}, minmod + HLL, CFL 0.5 (BASELINE configs[0] at n=1000, "
+             "kn=0.01): a correctness config, far too small to load a GPU (launch-latency bound)"),
+    "sod14": (lambda n, kn: wl.sod14(n, 4, Kn=kn), 0.5,
+              "14-moment Sod tube on {n}x4 cells, periodic y, Kn={kn}, minmod + HLL, CFL 0.5 (BASELINE configs[1] "
+              "at n=4096): a correctness config, 16 K cells"),
 }
 WORKLOAD = "baseline"
 
@@ -149,7 +155,7 @@ def time_oracle(n: int, kn: float, steps: int, warmup: int = 0, nthreads: int = 
     t0 = time.perf_counter()
     so.step(steps, CFL)
     dt = time.perf_counter() - t0
-    return n * n * steps / dt, so.threads, dt
+    return prob["nx"] * prob["ny"] * steps / dt, so.threads, dt
 
 
 def run_reference(args):
@@ -192,11 +198,12 @@ def run_gpu(args):
 
     n, K, W = args.n, args.steps, args.warmup
     prob = workload(n, args.kn)
-    cells = n * n
+    nm = prob["system"]
+    cells = prob["nx"] * prob["ny"]
     s = mm.Solver.from_problem(prob, load_state=False, device=f"cuda:{local}")
-    nbytes_state = 14 * cells * 8
+    nbytes_state = nm * cells * 8
     W_host = torch.from_numpy(prob["W0"]).pin_memory()
-    U_host = torch.empty((14, n, n), dtype=torch.float64).pin_memory()
+    U_host = torch.empty((nm, prob["ny"], prob["nx"]), dtype=torch.float64).pin_memory()
     W_dev = W_host.to(f"cuda:{local}")
 
     if args.general_path:
@@ -236,12 +243,12 @@ def run_gpu(args):
     finite = bool(torch.isfinite(U_host).all())
 
     if rank == 0:
-        fpc, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]), s.fast_path_active)
+        fpc, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]), s.fast_path_active, nm)
         peak_tf = mm.mm_measure_fp64_peak(5)
         kern_avg_ms = kern_ms / max(kern_n, 1)
         achieved_tf = fpc * cells / (kern_avg_ms * 1e-3) * 1e-12
         pk = peaks()
-        hbm_gbs = 224.0 * cells / (kern_avg_ms * 1e-3) * 1e-9
+        hbm_gbs = 16.0 * nm * cells / (kern_avg_ms * 1e-3) * 1e-9
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             v, threads, secs = time_oracle(args.ref_n, args.kn, args.cpu_steps)
@@ -249,11 +256,13 @@ def run_gpu(args):
                    "sample": f"{args.ref_n}x{args.ref_n} instance of the same workload, "
                              f"{args.cpu_steps} CFL steps ({secs:.1f} s)"}
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "metric": METRIC if nm == 14 else "cell-updates/s (fp64, 5-moment 1-D)",
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOADS[WORKLOAD][2].format(n=n, kn=args.kn),
-                       "cells": cells, "l2": f"inputs larger than L2 (2 x {nbytes_state / 1e6:.0f} MB state copies)",
+                       "cells": cells, "l2": (f"inputs larger than L2 (2 x {nbytes_state / 1e6:.0f} MB state copies)" if nbytes_state > 126e6
+                              else f"L2-resident state ({nbytes_state / 1e6:.2f} MB): not a bandwidth measurement"),
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "t_end": info["t"], "state_finite": finite},
             "clocks": clk.summary(),
@@ -264,7 +273,8 @@ def run_gpu(args):
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved_tf / peak_tf if peak_tf else None, "traffic": None,
-                         "kernel": "k_step14_strip<zsym>" if s.fast_path_active else "k_step14_strip<general>",
+                         "kernel": ("k_step5" if nm == 5 else
+                                    "k_step14_strip<zsym>" if s.fast_path_active else "k_step14_strip<general>"),
                          "kernel_ms": kern_avg_ms,
                          "flops_per_cell_update": fpc, "flops_per_cell_update_oracle": fpc_oracle,
                          "peak_source": "FP64 DFMA loop measured in this run (mm_measure_fp64_peak)",
