@@ -89,7 +89,7 @@ typedef struct {
 } mm_options;
 
 /* Bytes of device workspace mm_create needs for this grid (two padded state copies, boundary
- * tables, control block).  0 on invalid grid. */
+ * tables, control block, wave-speed table, dt history).  0 on invalid grid. */
 size_t mm_workspace_bytes(const mm_grid *grid);
 
 /* Build a solver on caller-provided device memory.  d_workspace: DEVICE pointer. */
@@ -121,6 +121,15 @@ int mm_get_state_prim(mm_solver *s, double *W, int on_device);
 int mm_get_info(mm_solver *s, double *t, long long *steps, double *last_dt, double *max_speed);
 /* dt the next mm_step(., cfl) would take.  Synchronises. */
 int mm_cfl_dt(mm_solver *s, double cfl, double *dt);
+
+/* Time steps dt of the steps first_step .. first_step + n - 1 (0-based; Fig 14 plots this
+ * curve).  The library keeps the last 65536 on the device, so n steps can be enqueued without a host
+ * round trip per step.  `dt` is a host array.  MM_EINVAL if the range has not been taken yet or has
+ * been overwritten.  Synchronises. */
+int mm_get_dt_history(mm_solver *s, long long first_step, int n, double *dt);
+/* Restore the clock after mm_set_state* (which resets t and the step counter to 0): with
+ * mm_get_state + mm_get_info this makes mm_set_state + mm_set_clock a checkpoint / resume pair. */
+int mm_set_clock(mm_solver *s, double t, long long steps);
 
 /* Number of kernel launches enqueued by this solver so far. */
 long long mm_launch_count(const mm_solver *s);

@@ -28,11 +28,7 @@ constexpr int kBlocksByRegs = 8 / kStripWPB;
 constexpr int kBlocksGenSmem = (int)((227 * 1024) / (kSmemGen + 1024));
 constexpr int kBlocksZSSmem = (int)((227 * 1024) / (kSmemZS + 1024));
 constexpr int kMinBlocksGen = kBlocksGenSmem < kBlocksByRegs ? kBlocksGenSmem : kBlocksByRegs;
-#ifdef MM_ZS_MINB
-constexpr int kMinBlocksZS = MM_ZS_MINB;
-#else
 constexpr int kMinBlocksZS = kBlocksZSSmem < kBlocksByRegs ? kBlocksZSSmem : kBlocksByRegs;
-#endif
 
 thread_local char g_cuda_msg[256] = "";
 
@@ -40,7 +36,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
     int nm, pitch, rows;
-    size_t plane, state_bytes, off_ctrl, off_bc, off_tab, off_u0, off_u1, total;
+    size_t plane, state_bytes, off_ctrl, off_bc, off_tab, off_hist, off_u0, off_u1, total;
 };
 
 bool make_layout(const mm_grid* g, Layout* L)
@@ -58,7 +54,8 @@ bool make_layout(const mm_grid* g, Layout* L)
     L->off_ctrl = 0;
     L->off_bc = align_up(sizeof(Ctrl), 256);
     L->off_tab = L->off_bc + align_up(sizeof(BcTable), 256);
-    L->off_u0 = L->off_tab + align_up(AbTable::kDoubles * sizeof(double), 256);
+    L->off_hist = L->off_tab + align_up(AbTable::kDoubles * sizeof(double), 256);
+    L->off_u0 = L->off_hist + align_up((size_t)kDtHistory * sizeof(double), 256);
     L->off_u1 = L->off_u0 + L->state_bytes;
     L->total = L->off_u1 + L->state_bytes;
     return true;
@@ -123,7 +120,8 @@ int launch_ghost(mm_solver* s, const StepCtl& sc, int finalize)
 {
     const int n = 4 * s->p.ny + (NM == 5 ? 0 : 4 * s->p.nx);
     const int nt = 128, nb = (n + nt - 1) / nt;
-    k_ghost<NM><<<nb, nt, 0, s->stream>>>(s->p, s->U[s->cur], s->bc, s->ctrl, s->slot, sc, finalize);
+    k_ghost<NM><<<nb, nt, 0, s->stream>>>(s->p, s->U[s->cur], s->bc, s->ctrl, s->slot, sc, finalize,
+                                          (double*)(s->ws + s->L.off_hist));
     MM_LAUNCHED(s, "k_ghost");
     return MM_OK;
 }
@@ -459,6 +457,34 @@ int mm_cfl_dt(mm_solver* s, double cfl, double* dt)
     double rate = fmax(bits2d(h.rate_bits[s->slot]), h.ghost_rate);
     if (h.failed || h.bc_bad || h.bad[s->slot] || !(rate > 0.0)) return MM_ENONFINITE;
     *dt = cfl / rate;
+    return MM_OK;
+}
+
+int mm_get_dt_history(mm_solver* s, long long first_step, int n, double* dt)
+{
+    if (!s || !dt || n < 0 || first_step < 0) return MM_EINVAL;
+    if (n == 0) return MM_OK;
+    Ctrl h;
+    int rc = read_ctrl(s, &h);
+    if (rc) return rc;
+    if (first_step + n > h.steps || h.steps - first_step > kDtHistory) return MM_EINVAL;   // not taken yet / overwritten
+    const double* hist = (const double*)(s->ws + s->L.off_hist);
+    for (int k = 0; k < n;) {                      // the ring wraps at most once inside the range
+        const long long pos = (first_step + k) & (kDtHistory - 1);
+        const int run = (int)((long long)(n - k) < kDtHistory - pos ? (n - k) : kDtHistory - pos);
+        MM_CUDA(cudaMemcpyAsync(dt + k, hist + pos, (size_t)run * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        k += run;
+    }
+    MM_CUDA(cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
+
+int mm_set_clock(mm_solver* s, double t, long long steps)
+{
+    if (!s || !s->has_state || !(t >= 0.0) || steps < 0) return MM_EINVAL;
+    MM_CUDA(cudaMemcpyAsync(&s->ctrl->t, &t, sizeof t, cudaMemcpyHostToDevice, s->stream));
+    MM_CUDA(cudaMemcpyAsync(&s->ctrl->steps, &steps, sizeof steps, cudaMemcpyHostToDevice, s->stream));
+    MM_CUDA(cudaStreamSynchronize(s->stream));     // t and steps are stack variables
     return MM_OK;
 }
 

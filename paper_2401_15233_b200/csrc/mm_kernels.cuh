@@ -11,6 +11,7 @@
 namespace mm {
 
 constexpr int kMaxBands = 8;
+constexpr int kDtHistory = 1 << 16;     // time steps kept in the device-side dt history (ring)
 
 // Control block (device memory).  rate = max_cells max(s_x/dx, s_y/dy), speed = max_cells s_d.
 struct Ctrl {
@@ -179,7 +180,7 @@ struct StepCtl {
 // accumulator slot the step kernel will max-reduce the NEXT state into.
 template <int NM>
 __global__ void k_ghost(Params p, double* __restrict__ U, const BcTable* __restrict__ tab,
-                        Ctrl* ctrl, int slot, StepCtl sc, int finalize)
+                        Ctrl* ctrl, int slot, StepCtl sc, int finalize, double* __restrict__ dt_hist)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (finalize && tid == 0) {
@@ -194,7 +195,10 @@ __global__ void k_ghost(Params p, double* __restrict__ U, const BcTable* __restr
             else if (tn >= sc.t_end) { dt = sc.t_end - t; tn = sc.t_end; }
         }
         if (skip) dt = 0.0;
-        else { ctrl->t = tn; ctrl->steps += 1; ctrl->last_dt = dt; }
+        else {
+            dt_hist[ctrl->steps & (kDtHistory - 1)] = dt;     // step number `steps` (0-based) took dt
+            ctrl->t = tn; ctrl->steps += 1; ctrl->last_dt = dt;
+        }
         ctrl->dt = dt;
         ctrl->skip = skip;
         // a skipped step carries the state over unchanged, and its reduction with it

@@ -65,11 +65,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // dt_scale = 1, do_rate = 1, source_scheme = 0 folded at compile time); EXT = true takes them at
 // run time (midpoint passes, point-implicit source).
 template <bool ZS, int MINB, bool EXT>
-#ifdef MM_MAXNREG
-__global__ void __maxnreg__(MM_MAXNREG)
-#else
 __global__ void __launch_bounds__(32 * kStripWPB, MINB)
-#endif
 k_step14_strip(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl,
                int slot_next, int nstrips, int nchunks, const double* Ubase_, double dt_scale_, int do_rate_)
 {

@@ -25,7 +25,7 @@ MAX_BANDS = 8
 
 EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim", "mm_step",
            "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
-           "mm_cfl_dt", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
+           "mm_cfl_dt", "mm_get_dt_history", "mm_set_clock", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
            "mm_measure_fp64_peak", "mm_selftest_fastmath", "mm_set_fast_path", "mm_fast_path_active",
            "mm_destroy", "mm_strerror"]
 
@@ -83,6 +83,8 @@ def lib() -> C.CDLL:
     L.mm_get_info.restype = i
     L.mm_get_info.argtypes = [vp, _dp, C.POINTER(C.c_longlong), _dp, _dp]
     L.mm_cfl_dt.restype, L.mm_cfl_dt.argtypes = i, [vp, d, _dp]
+    L.mm_get_dt_history.restype, L.mm_get_dt_history.argtypes = i, [vp, C.c_longlong, i, _dp]
+    L.mm_set_clock.restype, L.mm_set_clock.argtypes = i, [vp, d, C.c_longlong]
     L.mm_launch_count.restype, L.mm_launch_count.argtypes = C.c_longlong, [vp]
     L.mm_profile_begin.restype, L.mm_profile_begin.argtypes = i, [vp]
     L.mm_profile_end.restype = i
@@ -256,6 +258,16 @@ class Solver:
             _check(rc)
         return {"t": t.value, "steps": n.value, "last_dt": dt.value, "max_speed": sp.value,
                 "status": rc}
+
+    def dt_history(self, first_step: int, n: int) -> np.ndarray:
+        """dt of the steps first_step .. first_step + n - 1 (kept on the device, last 65536 steps)."""
+        out = np.empty(n, dtype=np.float64)
+        _check(self._L.mm_get_dt_history(self._h, first_step, n, out.ctypes.data_as(_dp)))
+        return out
+
+    def set_clock(self, t: float, steps: int):
+        """Restore t and the step counter after set_state (checkpoint / resume)."""
+        _check(self._L.mm_set_clock(self._h, t, steps))
 
     def profile_begin(self):
         _check(self._L.mm_profile_begin(self._h))

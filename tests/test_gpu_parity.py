@@ -448,6 +448,32 @@ def test_paper_crossing_jets_time_step_drop(mm):
     assert ratio[-3:].max() < 0.5                            # steps 3000 .. 3200: after the interaction
 
 
+def test_dt_history_and_checkpoint_resume(mm, mmo):
+    """The device-side dt history equals the oracle's step-by-step dt (Fig 14 is this
+    curve), and get_state + info / set_state + set_clock resume a run bit for bit."""
+    prob = wl.crossed_jets(64, Kn=1.0)
+    sg = mm.Solver.from_problem(prob); so = oracle_solver(mmo, prob)
+    sg.step(60, 0.4)
+    hist = sg.dt_history(0, 60)
+    ref = []
+    for _ in range(60):
+        so.step(1, 0.4); ref.append(so.info()["last_dt"])
+    assert np.allclose(hist, ref, rtol=1e-9, atol=0)
+    assert hist.sum() == pytest.approx(sg.info()["t"], rel=1e-13)
+    assert np.array_equal(sg.dt_history(57, 3), hist[57:])
+    with pytest.raises(mm.MMError):
+        sg.dt_history(58, 5)                                    # steps 60.. not taken yet
+    # checkpoint after 60 steps, 20 more; resume a fresh solver from the checkpoint, 20 more
+    U60, inf = sg.get_state(), sg.info()
+    sg.step(20, 0.4)
+    s2 = mm.Solver.from_problem(prob, load_state=False)
+    s2.set_state(U60); s2.set_clock(inf["t"], inf["steps"])
+    s2.step(20, 0.4)
+    assert np.array_equal(s2.get_state(), sg.get_state())
+    assert s2.info()["t"] == sg.info()["t"] and s2.info()["steps"] == 80
+    assert np.array_equal(s2.dt_history(60, 20), sg.dt_history(60, 20))
+
+
 # ------------------------------------------------------------------------ error behaviour
 def test_errors_and_failure_flag(mm, mmo):
     with pytest.raises(mm.MMError) as e:
