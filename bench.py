@@ -50,6 +50,13 @@ def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14):
     return float(k), o
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
+# `ncu --set full` capture summarised in profiles/ (None where no capture of that configuration exists).
+NCU_TRAFFIC_BYTES = {
+    ("k_step14_strip<zsym>", 2048): (352.04e6 + 423.10e6, "profiles/r1h_k_step14_strip_zsym.md"),
+}
+
+
 def peaks() -> dict:
     f = ROOT / "MEASURED_PEAKS.json"
     return json.loads(f.read_text()) if f.exists() else {}
@@ -255,6 +262,9 @@ def run_gpu(args):
             cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                    "sample": f"{args.ref_n}x{args.ref_n} instance of the same workload, "
                              f"{args.cpu_steps} CFL steps ({secs:.1f} s)"}
+        kernel_name = ("k_step5" if nm == 5 else
+                       "k_step14_strip<zsym>" if s.fast_path_active else "k_step14_strip<general>")
+        traffic, traffic_src = NCU_TRAFFIC_BYTES.get((kernel_name, n), (None, None)) if WORKLOAD == "baseline" else (None, None)
         out = {
             "metric": METRIC if nm == 14 else "cell-updates/s (fp64, 5-moment 1-D)",
             "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -272,9 +282,10 @@ def run_gpu(args):
                             f"D2H of the result; bytes amortised over the {K} steps"},
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                         "frac": achieved_tf / peak_tf if peak_tf else None, "traffic": None,
-                         "kernel": ("k_step5" if nm == 5 else
-                                    "k_step14_strip<zsym>" if s.fast_path_active else "k_step14_strip<general>"),
+                         "frac": achieved_tf / peak_tf if peak_tf else None,
+                         "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read + write)",
+                         "traffic_source": traffic_src, "algorithmic_bytes_per_launch": 16.0 * nm * cells,
+                         "kernel": kernel_name,
                          "kernel_ms": kern_avg_ms,
                          "flops_per_cell_update": fpc, "flops_per_cell_update_oracle": fpc_oracle,
                          "peak_source": "FP64 DFMA loop measured in this run (mm_measure_fp64_peak)",
