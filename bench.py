@@ -183,6 +183,55 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+def run_gpu_batch5(args):
+    """--workload sod5-batch: `--tubes` independent 5-moment Sod tubes of `--n` cells, sigma_lim x Kn
+    sweep values cycled over the tubes (section 4.3).  Single GPU."""
+    import torch
+    from paper_2401_15233_b200 import mm
+    torch.cuda.set_device(0)
+    nx, nt, K, W = args.n, args.tubes, args.steps, args.warmup
+    sig = np.resize([1e-2, 1e-3, 1e-4, 1e-5], nt)
+    kns = np.resize(np.repeat([1e-3, 1e-2, 1e-1, 1.0, 0.0], 4), nt)
+    W0 = wl.sod5(nx, Kn=0.01)["W0"].reshape(5, nx)
+    b = mm.Batch5(nx, sig, kns)
+    cells = nx * nt
+    b.set_state_prim(W0)
+    b.step(W, 0.5)
+    torch.cuda.synchronize()
+    l0 = b.launches
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(0) as clk:
+        ev0.record(); b.step(K, 0.5); ev1.record()
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    launches = b.launches - l0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); b.set_state_prim(W0); b.step(K, 0.5); U = b.get_state(); e1.record()
+    torch.cuda.synchronize()
+    e2e_ms = e0.elapsed_time(e1)
+    from paper_2401_15233_b200 import build_ext
+    fpc = float(build_ext.read_opcount()["kernel_flops_per_cell_update_5_per_variable_limiter"])
+    peak_tf = mm.mm_measure_fp64_peak(5)
+    achieved = fpc * cells * K / (ms * 1e-3) * 1e-12          # finalize kernel (ntubes threads) included
+    inf = b.info(check=False)
+    print(json.dumps({
+        "metric": "cell-updates/s (fp64, 5-moment 1-D, batched tubes)", "value": cells * K / (ms * 1e-3),
+        "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{nt} independent 5-moment Sod tubes x {nx} cells, sigma_lim in 1e-2..1e-5, Kn in "
+                               f"1e-3..1 and collisionless, minmod + HLL, own CFL 0.5 time step per tube "
+                               f"(SURVEY 8(f) item 4; not the BASELINE metric's workload)",
+                   "cells": cells, "state_finite": bool(np.isfinite(U).all()), "tubes_failed": int(inf["failed"].sum())},
+        "clocks": clk.summary(),
+        "e2e": {"value": cells * K / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": W0.nbytes / K,
+                "d2h_bytes_per_step": U.nbytes / K},
+        "gpu_launches": launches,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+                     "frac": achieved / peak_tf, "traffic": None, "kernel": "k_batch5_step",
+                     "flops_per_cell_update": fpc},
+        "cpu_baseline": None}), flush=True)
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -310,12 +359,15 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=250,
                     help="oracle steps of the cpu_baseline leg (~15 s on 16 cores at 512^2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="baseline", choices=sorted(WORKLOADS),
+    ap.add_argument("--tubes", type=int, default=4096, help="--workload sod5-batch: number of tubes")
+    ap.add_argument("--workload", default="baseline", choices=sorted(WORKLOADS) + ["sod5-batch"],
                     help="baseline = BASELINE.json configs[3] (the metric); paper-* = the paper's own jet cases")
     ap.add_argument("--general-path", action="store_true",
                     help="forbid the z-symmetric kernel variant (measurement of the general one)")
     args = ap.parse_args()
     global WORKLOAD, CFL
+    if args.workload == "sod5-batch":
+        return run_gpu_batch5(args)
     WORKLOAD = args.workload
     CFL = WORKLOADS[WORKLOAD][1]
     if args.impl == "reference":

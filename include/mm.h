@@ -161,6 +161,31 @@ int mm_measure_fp64_peak(void *stream, int repeats, double *tflops);
  *     pow / exp (whose own conditioning, P*^2 eps in the exponent, is ~10 units at P* = 3). */
 int mm_selftest_fastmath(void *stream, int n, double max_ulp[3]);
 
+/* ---- Batched 1-D 5-moment solver: `ntubes` independent shock tubes
+ * of nx cells on [x0, x1], transmissive ends (L426), each with its own sigma_lim (L163) and Knudsen
+ * number (tau = Kn L_ref (rho_ref/rho)/sqrt(8P/(pi rho)), L284; Kn <= 0: collisionless), its own CFL
+ * time step (L434) and clock -- the sigma_lim x Kn sweep of PAPER.md section 4.3 (L340-356, Fig 7) as
+ * one launch sequence.  Same scheme as MM_SYS5_1D (Eq 12, 14, 15, 34-35; forward Euler, explicit
+ * source).  sigma_lim and Kn are host arrays [ntubes], copied at create; workspace rules as mm_create.
+ * States: W primitives [5][nx] (one tube, copied to all; per_tube = 0) or [ntubes][5][nx];
+ * U conserved [ntubes][5][nx].  mm_batch5_advance_to steps until every tube has reached t_end (each
+ * lands on it exactly and then idles) or max_steps (> 0) steps were taken; the per-tube step counts
+ * of mm_batch5_get_info are the paper's measure of computational cost (L342).  failed[j] != 0 and
+ * MM_ENONFINITE when a tube's CFL reduction met rho <= 0, P <= 0 or a non-finite speed. */
+typedef struct mm_batch5 mm_batch5;
+size_t mm_batch5_workspace_bytes(int nx, int ntubes);
+int mm_batch5_create(mm_batch5 **out, int nx, int ntubes, double x0, double x1, const double *sigma_lim,
+                     const double *Kn, double L_ref, double rho_ref, double ws_scale, int limiter,
+                     int shared_limiter, int flux, void *stream, void *d_workspace, size_t bytes);
+int mm_batch5_set_state_prim(mm_batch5 *b, const double *W, int per_tube, int on_device);
+int mm_batch5_step(mm_batch5 *b, int n, double cfl);
+int mm_batch5_step_fixed_dt(mm_batch5 *b, int n, double dt);
+int mm_batch5_advance_to(mm_batch5 *b, double t_end, double cfl, long long max_steps);
+int mm_batch5_get_state(mm_batch5 *b, double *U, int on_device);
+int mm_batch5_get_info(mm_batch5 *b, double *t, long long *steps, int *failed);
+long long mm_batch5_launch_count(const mm_batch5 *b);
+void mm_batch5_destroy(mm_batch5 *b);
+
 void mm_destroy(mm_solver *s);
 const char *mm_strerror(int status);
 

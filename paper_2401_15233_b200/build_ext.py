@@ -10,7 +10,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libmm.so"
 SOURCES = ["mm_api.cu"]
-DEPS = ["mm_api.cu", "mm_kernels.cuh", "mm_strip14.cuh", "mm_physics.cuh", "../../include/mm.h"]
+DEPS = ["mm_api.cu", "mm_kernels.cuh", "mm_strip14.cuh", "mm_batch5.cuh", "mm_physics.cuh", "../../include/mm.h"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]
 

@@ -3,6 +3,7 @@
 #include "../../include/mm.h"
 #include "mm_kernels.cuh"
 #include "mm_strip14.cuh"
+#include "mm_batch5.cuh"
 
 #include <cstdio>
 #include <cstring>
@@ -575,6 +576,189 @@ int mm_selftest_fastmath(void* stream, int n, double* max_ulp)
     for (int k = 0; k < 3; ++k) max_ulp[k] = bits2d(h[k]);
     return MM_OK;
 }
+
+// ---------------------------------------------------------------- batched 1-D 5-moment tubes
+struct mm_batch5 {
+    int nx, ntubes;
+    Params p;
+    cudaStream_t stream;
+    char* ws;
+    TubeCtl* ctl;
+    double *sigma_lim, *inv_tau_coef, *U[2];
+    size_t state_bytes;
+    int cur, slot, has_state;
+    long long launches;
+};
+
+namespace {
+constexpr int kNTB = 128;
+struct BLayout { size_t off_ctl, off_sig, off_itc, off_u0, off_u1, state_bytes, total; };
+bool batch_layout(int nx, int ntubes, BLayout* L)
+{
+    if (nx < 1 || ntubes < 1 || ntubes > 65535) return false;
+    L->state_bytes = align_up((size_t)ntubes * 5 * nx * sizeof(double), 256);
+    L->off_ctl = 0;
+    L->off_sig = align_up((size_t)ntubes * sizeof(TubeCtl), 256);
+    L->off_itc = L->off_sig + align_up((size_t)ntubes * sizeof(double), 256);
+    L->off_u0 = L->off_itc + align_up((size_t)ntubes * sizeof(double), 256);
+    L->off_u1 = L->off_u0 + L->state_bytes;
+    L->total = L->off_u1 + L->state_bytes;
+    return true;
+}
+int batch_step(mm_batch5* b, const StepCtl& sc)
+{
+    k_batch5_finalize<<<(b->ntubes + 127) / 128, 128, 0, b->stream>>>(b->ntubes, b->ctl, b->slot, sc);
+    dim3 grid((b->nx + kNTB - 1) / kNTB, b->ntubes);
+    k_batch5_step<kNTB><<<grid, kNTB, 0, b->stream>>>(b->p, b->sigma_lim, b->inv_tau_coef, b->U[b->cur],
+                                                     b->U[b->cur ^ 1], b->ctl, b->slot ^ 1);
+    b->launches += 2;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "k_batch5_step");
+    b->cur ^= 1; b->slot ^= 1;
+    return MM_OK;
+}
+int batch_read_ctl(mm_batch5* b, std::vector<TubeCtl>& h)
+{
+    h.resize(b->ntubes);
+    MM_CUDA(cudaMemcpyAsync(h.data(), b->ctl, (size_t)b->ntubes * sizeof(TubeCtl), cudaMemcpyDeviceToHost, b->stream));
+    MM_CUDA(cudaStreamSynchronize(b->stream));
+    return MM_OK;
+}
+}  // namespace
+
+size_t mm_batch5_workspace_bytes(int nx, int ntubes)
+{
+    BLayout L;
+    return batch_layout(nx, ntubes, &L) ? L.total : 0;
+}
+
+int mm_batch5_create(mm_batch5** out, int nx, int ntubes, double x0, double x1, const double* sigma_lim,
+                     const double* Kn, double L_ref, double rho_ref, double ws_scale, int limiter,
+                     int shared_limiter, int flux, void* stream, void* d_workspace, size_t bytes)
+{
+    if (!out || !sigma_lim || !Kn || !(x1 > x0) || !(ws_scale > 0.0) || !(L_ref > 0.0) || !(rho_ref > 0.0)) return MM_EINVAL;
+    if (limiter < 0 || limiter > 2 || flux < 0 || flux > 1) return MM_EINVAL;
+    BLayout L;
+    if (!batch_layout(nx, ntubes, &L)) return MM_EINVAL;
+    for (int j = 0; j < ntubes; ++j) if (!(sigma_lim[j] > 0.0)) return MM_EINVAL;
+    if (!d_workspace || bytes < L.total || ((size_t)d_workspace & 255)) return MM_EWORKSPACE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return cuda_fail(cudaErrorNoDevice, "mm_batch5_create (no CUDA device: this library has no CPU path)");
+    mm_batch5* b = new (std::nothrow) mm_batch5();
+    if (!b) return MM_EINVAL;
+    b->nx = nx; b->ntubes = ntubes; b->stream = (cudaStream_t)stream; b->ws = (char*)d_workspace;
+    b->ctl = (TubeCtl*)(b->ws + L.off_ctl);
+    b->sigma_lim = (double*)(b->ws + L.off_sig); b->inv_tau_coef = (double*)(b->ws + L.off_itc);
+    b->U[0] = (double*)(b->ws + L.off_u0); b->U[1] = (double*)(b->ws + L.off_u1);
+    b->state_bytes = L.state_bytes;
+    Params& p = b->p;
+    memset(&p, 0, sizeof p);
+    p.ws_scale = ws_scale; p.dx = (x1 - x0) / nx; p.dy = 1.0; p.x0 = x0;
+    p.limiter = limiter; p.shared_limiter = shared_limiter ? 1 : 0; p.flux = flux;
+    p.nx = nx; p.ny = 1;
+    std::vector<double> itc(ntubes);
+    for (int j = 0; j < ntubes; ++j) itc[j] = Kn[j] > 0.0 ? 1.0 / (Kn[j] * L_ref * rho_ref) : 0.0;   // <= 0: collisionless
+    cudaError_t e = cudaMemsetAsync(b->ws, 0, L.off_u0, b->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(b->sigma_lim, sigma_lim, ntubes * sizeof(double), cudaMemcpyHostToDevice, b->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(b->inv_tau_coef, itc.data(), ntubes * sizeof(double), cudaMemcpyHostToDevice, b->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
+    if (e != cudaSuccess) { delete b; return cuda_fail(e, "mm_batch5_create"); }
+    *out = b;
+    return MM_OK;
+}
+
+int mm_batch5_set_state_prim(mm_batch5* b, const double* W, int per_tube, int on_device)
+{
+    if (!b || !W) return MM_EINVAL;
+    const size_t nbytes = (size_t)(per_tube ? b->ntubes : 1) * 5 * b->nx * sizeof(double);
+    const double* src = W;
+    if (!on_device) {
+        MM_CUDA(cudaMemcpyAsync(b->U[b->cur ^ 1], W, nbytes, cudaMemcpyHostToDevice, b->stream));
+        src = b->U[b->cur ^ 1];
+    }
+    dim3 grid((b->nx + 127) / 128, b->ntubes);
+    k_batch5_pack<<<grid, 128, 0, b->stream>>>(b->nx, b->ntubes, per_tube ? 1 : 0, src, b->U[b->cur]);
+    MM_CUDA(cudaMemsetAsync(b->ctl, 0, (size_t)b->ntubes * sizeof(TubeCtl), b->stream));
+    b->slot = 0;
+    dim3 g2((b->nx + kNTB - 1) / kNTB, b->ntubes);
+    k_batch5_rate<kNTB><<<g2, kNTB, 0, b->stream>>>(b->p, b->sigma_lim, b->inv_tau_coef, b->U[b->cur], b->ctl);
+    b->launches += 2;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "mm_batch5_set_state_prim");
+    b->has_state = 1;
+    return MM_OK;
+}
+
+int mm_batch5_step(mm_batch5* b, int n, double cfl)
+{
+    if (!b || n < 0 || !(cfl > 0.0) || !b->has_state) return MM_EINVAL;
+    StepCtl sc = {1, cfl, -1.0};
+    for (int k = 0; k < n; ++k) { int rc = batch_step(b, sc); if (rc) return rc; }
+    return MM_OK;
+}
+
+int mm_batch5_step_fixed_dt(mm_batch5* b, int n, double dt)
+{
+    if (!b || n < 0 || !(dt > 0.0) || !b->has_state) return MM_EINVAL;
+    StepCtl sc = {0, dt, -1.0};
+    for (int k = 0; k < n; ++k) { int rc = batch_step(b, sc); if (rc) return rc; }
+    return MM_OK;
+}
+
+int mm_batch5_advance_to(mm_batch5* b, double t_end, double cfl, long long max_steps)
+{
+    if (!b || !(cfl > 0.0) || !(t_end >= 0.0) || !b->has_state) return MM_EINVAL;
+    StepCtl sc = {1, cfl, t_end};
+    std::vector<TubeCtl> h;
+    long long done = 0;
+    for (;;) {
+        int rc = batch_read_ctl(b, h);
+        if (rc) return rc;
+        double need = 0.0;                      // steps the slowest unfinished tube still needs, estimated
+        for (const TubeCtl& c : h) {
+            if (c.failed || c.t >= t_end) continue;
+            const double rate = bits2d(c.rate_bits[b->slot]);
+            const double est = rate > 0.0 ? (t_end - c.t) * rate / cfl : 1.0;
+            if (est > need) need = est;
+        }
+        if (need <= 0.0 || (max_steps > 0 && done >= max_steps)) break;
+        long long batch = need < 1.0 ? 1 : (need > 512.0 ? 512 : (long long)need + 1);
+        if (max_steps > 0 && batch > max_steps - done) batch = max_steps - done;
+        for (long long k = 0; k < batch; ++k) if ((rc = batch_step(b, sc))) return rc;
+        done += batch;
+    }
+    return MM_OK;
+}
+
+int mm_batch5_get_state(mm_batch5* b, double* U, int on_device)
+{
+    if (!b || !U || !b->has_state) return MM_EINVAL;
+    const size_t nbytes = (size_t)b->ntubes * 5 * b->nx * sizeof(double);
+    MM_CUDA(cudaMemcpyAsync(U, b->U[b->cur], nbytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, b->stream));
+    MM_CUDA(cudaStreamSynchronize(b->stream));
+    return MM_OK;
+}
+
+int mm_batch5_get_info(mm_batch5* b, double* t, long long* steps, int* failed)
+{
+    if (!b) return MM_EINVAL;
+    std::vector<TubeCtl> h;
+    int rc = batch_read_ctl(b, h);
+    if (rc) return rc;
+    int any = 0;
+    for (int j = 0; j < b->ntubes; ++j) {
+        const int f = h[j].failed || h[j].bad[b->slot];
+        if (t) t[j] = h[j].t;
+        if (steps) steps[j] = h[j].steps;
+        if (failed) failed[j] = f;
+        any |= f;
+    }
+    return any ? MM_ENONFINITE : MM_OK;
+}
+
+long long mm_batch5_launch_count(const mm_batch5* b) { return b ? b->launches : 0; }
+void mm_batch5_destroy(mm_batch5* b) { delete b; }
 
 void mm_destroy(mm_solver* s)
 {

@@ -27,7 +27,10 @@ EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim
            "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
            "mm_cfl_dt", "mm_get_dt_history", "mm_set_clock", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
            "mm_measure_fp64_peak", "mm_selftest_fastmath", "mm_set_fast_path", "mm_fast_path_active",
-           "mm_destroy", "mm_strerror"]
+           "mm_destroy", "mm_strerror",
+           "mm_batch5_workspace_bytes", "mm_batch5_create", "mm_batch5_set_state_prim", "mm_batch5_step",
+           "mm_batch5_step_fixed_dt", "mm_batch5_advance_to", "mm_batch5_get_state", "mm_batch5_get_info",
+           "mm_batch5_launch_count", "mm_batch5_destroy"]
 
 _dp = C.POINTER(C.c_double)
 
@@ -94,6 +97,18 @@ def lib() -> C.CDLL:
     L.mm_set_fast_path.restype, L.mm_set_fast_path.argtypes = i, [vp, i]
     L.mm_fast_path_active.restype, L.mm_fast_path_active.argtypes = i, [vp]
     L.mm_destroy.restype, L.mm_destroy.argtypes = None, [vp]
+    L.mm_batch5_workspace_bytes.restype, L.mm_batch5_workspace_bytes.argtypes = C.c_size_t, [i, i]
+    L.mm_batch5_create.restype = i
+    L.mm_batch5_create.argtypes = [C.POINTER(vp), i, i, d, d, _dp, _dp, d, d, d, i, i, i, vp, vp, C.c_size_t]
+    L.mm_batch5_set_state_prim.restype, L.mm_batch5_set_state_prim.argtypes = i, [vp, vp, i, i]
+    L.mm_batch5_step.restype, L.mm_batch5_step.argtypes = i, [vp, i, d]
+    L.mm_batch5_step_fixed_dt.restype, L.mm_batch5_step_fixed_dt.argtypes = i, [vp, i, d]
+    L.mm_batch5_advance_to.restype, L.mm_batch5_advance_to.argtypes = i, [vp, d, d, C.c_longlong]
+    L.mm_batch5_get_state.restype, L.mm_batch5_get_state.argtypes = i, [vp, vp, i]
+    L.mm_batch5_get_info.restype = i
+    L.mm_batch5_get_info.argtypes = [vp, _dp, C.POINTER(C.c_longlong), C.POINTER(C.c_int)]
+    L.mm_batch5_launch_count.restype, L.mm_batch5_launch_count.argtypes = C.c_longlong, [vp]
+    L.mm_batch5_destroy.restype, L.mm_batch5_destroy.argtypes = None, [vp]
     L.mm_strerror.restype, L.mm_strerror.argtypes = C.c_char_p, [i]
     _lib = L
     return L
@@ -308,3 +323,79 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+
+class Batch5:
+    """mm_batch5_*: `ntubes` independent 1-D 5-moment tubes with per-tube sigma_lim and Kn
+    (include/mm.h).  Kn <= 0 or None marks a collisionless tube."""
+
+    def __init__(self, nx, sigma_lim, Kn, extent=(0.0, 1.0), L_ref=1.0, rho_ref=1.0, ws_scale=1.0,
+                 limiter=LIM_MINMOD, shared_limiter=0, flux=FLUX_HLL, device="cuda:0", stream=None):
+        import torch
+        L = lib()
+        self._L, self._h = L, None
+        sig = _darr(sigma_lim)
+        kn = _darr([k if k is not None else 0.0 for k in Kn])
+        if sig.size != kn.size:
+            raise ValueError("sigma_lim and Kn must have one entry per tube")
+        self.nx, self.ntubes = nx, sig.size
+        nbytes = L.mm_batch5_workspace_bytes(nx, self.ntubes)
+        if nbytes == 0:
+            raise MMError(EINVAL, "invalid batch")
+        if not torch.cuda.is_available():
+            raise MMError(ECUDA, "no CUDA device: this library has no CPU path")
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self._stream = stream if stream is not None else torch.cuda.current_stream()
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+            h = C.c_void_p()
+            _check(L.mm_batch5_create(C.byref(h), nx, self.ntubes, extent[0], extent[1],
+                                      sig.ctypes.data_as(_dp), kn.ctypes.data_as(_dp), L_ref, rho_ref, ws_scale,
+                                      limiter, shared_limiter, flux, C.c_void_p(self._stream.cuda_stream),
+                                      C.c_void_p(ptr), nbytes))
+            self._h = h
+
+    def set_state_prim(self, W):
+        """W: numpy [5][nx] (copied to every tube) or [ntubes][5][nx]."""
+        a = np.ascontiguousarray(W, dtype=np.float64)
+        per_tube = a.ndim == 3
+        if a.size != (self.ntubes if per_tube else 1) * 5 * self.nx:
+            raise ValueError("bad state shape")
+        _check(self._L.mm_batch5_set_state_prim(self._h, a.ctypes.data_as(C.c_void_p), int(per_tube), 0))
+
+    def step(self, n, cfl):
+        _check(self._L.mm_batch5_step(self._h, n, cfl))
+
+    def step_fixed_dt(self, n, dt):
+        _check(self._L.mm_batch5_step_fixed_dt(self._h, n, dt))
+
+    def advance_to(self, t_end, cfl, max_steps=0):
+        _check(self._L.mm_batch5_advance_to(self._h, t_end, cfl, max_steps))
+
+    def get_state(self):
+        out = np.empty((self.ntubes, 5, self.nx), dtype=np.float64)
+        _check(self._L.mm_batch5_get_state(self._h, out.ctypes.data_as(C.c_void_p), 0))
+        return out
+
+    def info(self, check=True):
+        t = np.empty(self.ntubes); n = np.empty(self.ntubes, dtype=np.int64); f = np.empty(self.ntubes, dtype=np.int32)
+        rc = self._L.mm_batch5_get_info(self._h, t.ctypes.data_as(_dp), n.ctypes.data_as(C.POINTER(C.c_longlong)),
+                                        f.ctypes.data_as(C.POINTER(C.c_int)))
+        if check:
+            _check(rc)
+        return {"t": t, "steps": n, "failed": f, "status": rc}
+
+    @property
+    def launches(self):
+        return self._L.mm_batch5_launch_count(self._h)
+
+    def sync(self):
+        import torch
+        torch.cuda.synchronize(self.device)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._L.mm_batch5_destroy(self._h)
+            self._h = None
+

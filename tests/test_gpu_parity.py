@@ -474,6 +474,96 @@ def test_dt_history_and_checkpoint_resume(mm, mmo):
     assert np.array_equal(s2.dt_history(60, 20), sg.dt_history(60, 20))
 
 
+# ------------------------------ batched 1-D 5-moment tubes (sigma_lim x Kn sweep)
+def _tube_oracles(mmo, nx, sigma_lims, Kns, **opt):
+    out = []
+    for sl, kn in zip(sigma_lims, Kns):
+        prob = wl.sod5(nx, Kn=kn, sigma_lim=sl, **opt)
+        out.append(oracle_solver(mmo, prob))
+    return out
+
+
+def test_batch5_matches_independent_oracle_tubes(mm, mmo):
+    """Every tube of a batch equals its own 1-D oracle run: different sigma_lim and Kn per tube
+    (one collisionless), 100 steps at a common fixed dt, then CFL stepping where every tube takes
+    its own dt and lands on t_end by itself."""
+    nx = 333
+    sig = [1e-4, 1e-3, 1e-2, 1e-4, 1e-5]
+    kns = [0.01, 0.1, 1.0, None, 0.001]
+    W0 = wl.sod5(nx, Kn=0.01)["W0"].reshape(5, nx)
+    b = mm.Batch5(nx, sig, kns)
+    b.set_state_prim(W0)
+    dt = 0.5 * min(scout_dt(mmo, wl.sod5(nx, Kn=kn, sigma_lim=sl), 100, 0.5) for sl, kn in zip(sig, kns))
+    tubes = _tube_oracles(mmo, nx, sig, kns)
+    b.step_fixed_dt(100, dt)
+    Ub = b.get_state()
+    for j, t in enumerate(tubes):
+        t.step_fixed_dt(100, dt)
+        assert_parity(Ub[j].reshape(5, 1, nx), t.get_state())
+    assert np.allclose(b.info()["t"], 100 * dt, rtol=1e-13)
+    # own CFL time steps, own clocks: element-wise over the first 30 steps ...
+    b.set_state_prim(W0)
+    tubes = _tube_oracles(mmo, nx, sig, kns)
+    b.step(30, 0.5)
+    inf = b.info()
+    Ub = b.get_state()
+    for j, t in enumerate(tubes):
+        t.step(30, 0.5)
+        assert inf["t"][j] == pytest.approx(t.info()["t"], rel=1e-9)
+        assert_parity(Ub[j].reshape(5, 1, nx), t.get_state(), 1e-8)
+    assert len(set(np.round(inf["t"], 12).tolist())) > 1       # the tubes really have their own clocks
+    # ... and to t_end through what is robust to round-off (DESIGN.md R24): every tube lands on t_end
+    # by itself, with a step count and a density profile close to its oracle's
+    b.advance_to(0.03, 0.5)
+    inf = b.info()
+    Ub = b.get_state()
+    for j, t in enumerate(tubes):
+        t.advance_to(0.03, 0.5)
+        assert inf["t"][j] == 0.03
+        assert abs(int(inf["steps"][j]) - t.info()["steps"]) <= 0.15 * t.info()["steps"]
+        rho_o = t.get_state()[0, 0]
+        assert np.abs(Ub[j, 0] - rho_o).mean() <= 5e-3 * rho_o.mean()
+    assert len(set(inf["steps"].tolist())) > 1
+
+
+def test_batch5_cost_rises_as_sigma_lim_falls(mm):
+    """PAPER.md L318-320, L350 (Fig 7-Left): a smaller sigma_lim lets the solution climb closer to the
+    Junk line, wave speeds grow and the run needs more time steps; collisions (small Kn) lower the cost
+    (L346).  64 tubes = 8 sigma_lim x 8 Kn in one batch, Sod tube to t = 0.1."""
+    nx = 500
+    sig = np.repeat([1e-1, 3e-2, 1e-2, 3e-3, 1e-3, 3e-4, 1e-4, 1e-5], 8)
+    kns = np.tile([1e-3, 3e-3, 1e-2, 3e-2, 1e-1, 0.3, 1.0, 0.0], 8)      # 0.0: collisionless
+    b = mm.Batch5(nx, sig, kns)
+    b.set_state_prim(wl.sod5(nx, Kn=0.01)["W0"].reshape(5, nx))
+    b.advance_to(0.1, 0.5)
+    inf = b.info()
+    assert np.all(inf["t"] == 0.1) and not inf["failed"].any()
+    steps = inf["steps"].reshape(8, 8)                           # [sigma_lim][Kn]
+    U = b.get_state()
+    assert np.all(np.isfinite(U)) and U[:, 0].min() > 0
+    collisionless = steps[:, 7]
+    assert np.all(np.diff(collisionless) >= 0) and collisionless[-1] > 3 * collisionless[0]
+    assert np.all(steps[6, :] >= steps[2, :])                    # sigma_lim 1e-4 never cheaper than 1e-2
+    assert steps[6, 0] < steps[6, 7]                             # Kn = 1e-3 cheaper than collisionless
+
+
+def test_batch5_errors(mm):
+    with pytest.raises(mm.MMError):
+        mm.Batch5(100, [1e-4, 0.0], [0.1, 0.1])                  # sigma_lim must be positive
+    with pytest.raises(ValueError):
+        mm.Batch5(100, [1e-4], [0.1, 0.2])
+    b = mm.Batch5(64, [1e-4, 1e-4], [0.1, 1.0])
+    with pytest.raises(mm.MMError):
+        b.step(1, 0.5)                                           # no state yet
+    W = wl.sod5(64, Kn=0.1)["W0"].reshape(5, 64).copy()
+    Wb = np.stack([W, W]); Wb[1, 2, 10] = -1.0                   # negative pressure in tube 1 only
+    b.set_state_prim(Wb)
+    b.step(5, 0.5)
+    inf = b.info(check=False)
+    assert inf["status"] == mm.ENONFINITE and list(inf["failed"]) == [0, 1]
+    assert inf["steps"][0] == 5 and inf["steps"][1] == 0        # the healthy tube keeps going
+
+
 # ------------------------------------------------------------------------ error behaviour
 def test_errors_and_failure_flag(mm, mmo):
     with pytest.raises(mm.MMError) as e:
