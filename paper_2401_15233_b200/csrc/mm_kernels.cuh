@@ -367,7 +367,7 @@ k_step5(Params p, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl, int 
                 double Wst[NM];
                 cons2prim5(Un, Wst);
                 const double x = dt * inv_tau(p, Wst[0], Wst[2]);
-                add_source5(Wst, x / (1.0 + x), Un);
+                add_source5(Wst, x * rcp(1.0 + x), Un);
             } else {
                 add_source5(W, dt * inv_tau(p, W[0], W[2]), Un);
             }

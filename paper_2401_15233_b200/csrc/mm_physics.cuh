@@ -162,7 +162,7 @@ struct PsiShared {
 // Eq 12 (L129-137).
 __device__ __forceinline__ void cons2prim5(const double (&U)[5], double (&W)[5])
 {
-    double rho = U[0], u = U[1] / rho;
+    double rho = U[0], u = U[1] * rcp(rho);
     double P = U[2] - rho * u * u;
     double q = U[3] - rho * u * u * u - 3.0 * u * P;
     double r = U[4] - rho * u * u * u * u - 6.0 * u * u * P - 4.0 * u * q;
@@ -182,8 +182,8 @@ __device__ __forceinline__ void prim2cons5(const double (&W)[5], double (&U)[5])
 __device__ __forceinline__ double sigma5(double qs, double rs)
 {
     double b = 3.0 - rs, X = qs * qs;
-    double D = sqrt(b * b + 8.0 * X);
-    return b >= 0.0 ? 0.25 * (b + D) : 2.0 * X / (D - b);
+    double D = fsqrt(b * b + 8.0 * X);
+    return b >= 0.0 ? 0.25 * (b + D) : 2.0 * X * rcp(D - b);
 }
 
 // Eq 34-35 (L543-551): lambda*_max(q*, sigma_bar); radicand floored at 0 (R6).
@@ -191,19 +191,19 @@ struct WS5 { double E, C, Y4, inv2s; };
 __device__ __forceinline__ WS5 ws5_common(double sb)
 {
     WS5 w;
-    double ss = sqrt(sb);
-    w.C = sqrt(3.0 - 3.0 * sb);
+    double ss = fsqrt(sb);
+    w.C = fsqrt(3.0 - 3.0 * sb);
     w.E = 0.8 * w.C;
-    double B = 5.0 - 4.0 * ss + sqrt(fmax(10.0 - 16.0 * ss + 6.0 * sb, 0.0));
-    double Y = B + w.E * w.E - 2.0 * w.E * sqrt(B);
+    double B = 5.0 - 4.0 * ss + fsqrt(dmax(10.0 - 16.0 * ss + 6.0 * sb, 0.0));
+    double Y = B + w.E * w.E - 2.0 * w.E * fsqrt(B);
     w.Y4 = 4.0 * sb * sb * Y;
-    w.inv2s = 0.5 / sb;
+    w.inv2s = 0.5 * rcp(sb);
     return w;
 }
 __device__ __forceinline__ double ws5_lambda(const WS5& w, double sb, double qs)
 {
-    double rad = fmax(qs * qs - 0.8 * qs * sb * w.C + w.Y4, 0.0);
-    return (qs + sqrt(rad)) * w.inv2s + w.E;
+    double rad = dmax(qs * qs - 0.8 * qs * sb * w.C + w.Y4, 0.0);
+    return (qs + fsqrt(rad)) * w.inv2s + w.E;
 }
 
 // min / max wave speed of a 5-moment state (Eqs 30, 31, 34).  ok = rho > 0 && P > 0.
@@ -211,8 +211,9 @@ __device__ __forceinline__ void wavespeed5(const Params& p, const double (&W)[5]
                                            double& lmax)
 {
     double rho = W[0], u = W[1], P = W[2], q = W[3], r = W[4];
-    double c2 = P / rho, c = sqrt(c2);
-    double qs = q / (rho * c2 * c), rs = r / (rho * c2 * c2);
+    double c2 = P * rcp(rho), c = fsqrt(c2);
+    double irc4 = rcp(rho * c2 * c2);                     // 1/(rho c^4); 1/(rho c^3) = c/(rho c^4)
+    double qs = q * (c * irc4), rs = r * irc4;
     double sb = clamp_sigma(sigma5(qs, rs), p.sigma_lim);
     WS5 w = ws5_common(sb);
     lmax = u + p.ws_scale * ws5_lambda(w, sb, qs) * c;
@@ -224,12 +225,13 @@ __device__ __forceinline__ void eval_face5(const Params& p, const double (&W)[5]
                                            double (&U)[5], double& lmin, double& lmax)
 {
     double rho = W[0], u = W[1], P = W[2], q = W[3], r = W[4];
-    double c2 = P / rho, c = sqrt(c2);
+    double c2 = P * rcp(rho), c = fsqrt(c2);
     double rc3 = rho * c2 * c;
-    double qs = q / rc3, rs = r / (rho * c2 * c2);
+    double irc4 = rcp(rc3 * c);
+    double qs = q * (c * irc4), rs = r * irc4;
     double sb = clamp_sigma(sigma5(qs, rs), p.sigma_lim);
     // Eq 15 (L155): s* = q*^3/sigma^2 + (10 - 8 sqrt(sigma)) q*;  s = rho c^5 s*
-    double s = rc3 * c2 * (qs * qs * qs / (sb * sb) + (10.0 - 8.0 * sqrt(sb)) * qs);
+    double s = rc3 * c2 * (qs * qs * qs * rcp(sb * sb) + (10.0 - 8.0 * fsqrt(sb)) * qs);
     prim2cons5(W, U);
     F[0] = U[1];
     F[1] = U[2];
@@ -247,14 +249,14 @@ __device__ __forceinline__ void add_source5(const double (&W)[5], double dt_over
 {
     double rho = W[0], u = W[1], P = W[2], q = W[3], r = W[4];
     Un[3] += dt_over_tau * (-q);
-    Un[4] += dt_over_tau * (-(4.0 * u * q + r - 3.0 * P * P / rho));
+    Un[4] += dt_over_tau * (-(4.0 * u * q + r - 3.0 * P * P * rcp(rho)));
 }
 __device__ __forceinline__ bool cell_speed5(const Params& p, const double (&W)[5], double& sx)
 {
     if (!(W[0] > 0.0) || !(W[2] > 0.0)) { sx = 0.0; return false; }
     double a, b;
     wavespeed5(p, W, a, b);
-    sx = fmax(fabs(a), fabs(b));
+    sx = dmax(fabs(a), fabs(b));
     return true;
 }
 
