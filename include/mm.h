@@ -131,6 +131,11 @@ int mm_get_dt_history(mm_solver *s, long long first_step, int n, double *dt);
  * mm_get_state + mm_get_info this makes mm_set_state + mm_set_clock a checkpoint / resume pair. */
 int mm_set_clock(mm_solver *s, double t, long long steps);
 
+/* Host logic only (no device needed): the work decomposition the 14-moment step kernel is launched
+ * with on a device of `sms` SMs -- strips of 30 cells in x times row chunks in y, one warp each,
+ * chosen to fill whole waves of sms * warps_per_sm resident warps. */
+int mm_decomposition(int nx, int ny, int zsym, int sms, int *nstrips, int *nchunks, int *warps_per_sm);
+
 /* Number of kernel launches enqueued by this solver so far. */
 long long mm_launch_count(const mm_solver *s);
 

@@ -491,6 +491,15 @@ int mm_set_clock(mm_solver* s, double t, long long steps)
 
 long long mm_launch_count(const mm_solver* s) { return s ? s->launches : 0; }
 
+int mm_decomposition(int nx, int ny, int zsym, int sms, int* nstrips, int* nchunks, int* warps_per_sm)
+{
+    if (nx < 1 || ny < 1 || sms < 1 || !nstrips || !nchunks || !warps_per_sm) return MM_EINVAL;
+    const int w = (zsym ? kMinBlocksZS : kMinBlocksGen) * kStripWPB;
+    choose_decomposition(nx, ny, sms * w, nstrips, nchunks);
+    *warps_per_sm = w;
+    return MM_OK;
+}
+
 int mm_set_fast_path(mm_solver* s, int allow)
 {
     if (!s) return MM_EINVAL;

@@ -25,7 +25,7 @@ MAX_BANDS = 8
 
 EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim", "mm_step",
            "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
-           "mm_cfl_dt", "mm_get_dt_history", "mm_set_clock", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
+           "mm_cfl_dt", "mm_get_dt_history", "mm_set_clock", "mm_decomposition", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
            "mm_measure_fp64_peak", "mm_selftest_fastmath", "mm_set_fast_path", "mm_fast_path_active",
            "mm_destroy", "mm_strerror",
            "mm_batch5_workspace_bytes", "mm_batch5_create", "mm_batch5_set_state_prim", "mm_batch5_step",
@@ -88,6 +88,8 @@ def lib() -> C.CDLL:
     L.mm_cfl_dt.restype, L.mm_cfl_dt.argtypes = i, [vp, d, _dp]
     L.mm_get_dt_history.restype, L.mm_get_dt_history.argtypes = i, [vp, C.c_longlong, i, _dp]
     L.mm_set_clock.restype, L.mm_set_clock.argtypes = i, [vp, d, C.c_longlong]
+    ip = C.POINTER(C.c_int)
+    L.mm_decomposition.restype, L.mm_decomposition.argtypes = i, [i, i, i, i, ip, ip, ip]
     L.mm_launch_count.restype, L.mm_launch_count.argtypes = C.c_longlong, [vp]
     L.mm_profile_begin.restype, L.mm_profile_begin.argtypes = i, [vp]
     L.mm_profile_end.restype = i
@@ -138,6 +140,13 @@ def mm_measure_fp64_peak(repeats: int = 5, stream=None) -> float:
     tf = C.c_double()
     _check(lib().mm_measure_fp64_peak(C.c_void_p(st.cuda_stream), repeats, C.byref(tf)))
     return tf.value
+
+
+def mm_decomposition(nx: int, ny: int, zsym: bool = True, sms: int = 148):
+    """-> (nstrips, nchunks, warps_per_sm) of the 14-moment step kernel's launch (host logic only)."""
+    a, b, c = C.c_int(), C.c_int(), C.c_int()
+    _check(lib().mm_decomposition(nx, ny, int(zsym), sms, C.byref(a), C.byref(b), C.byref(c)))
+    return a.value, b.value, c.value
 
 
 def mm_selftest_fastmath(n: int = 1 << 22, stream=None):

@@ -91,3 +91,24 @@ def test_product_does_not_touch_the_oracle():
         if f.suffix in (".py", ".cu", ".cuh", ".h"):
             assert "oracle" not in f.read_text().lower().replace("no cpu", ""), f
     assert "mmo" not in (ROOT / "include" / "mm.h").read_text()
+
+
+def test_launch_decomposition_host_logic(mm):
+    """Strips x row chunks of the 14-moment step kernel (no device needed): every cell is covered,
+    the items fill whole waves of the resident warps as well as the grid allows, and no chunk is empty."""
+    for nx, ny in [(2048, 2048), (4096, 4096), (512, 512), (1200, 1200), (4096, 4), (33, 9), (1, 1), (70, 37)]:
+        for zsym in (True, False):
+            ns, nc, w = mm.mm_decomposition(nx, ny, zsym, 148)
+            assert ns == -(-nx // 30) and 1 <= nc <= ny and w >= 6
+            slots = 148 * w
+            waves = -(-ns * nc // slots)
+            rows = -(-ny // nc)
+            # never worse than one chunk per strip, and within 15 % of the ideal split on large grids
+            assert waves * (rows + 0.8) <= -(-ns // slots) * (ny + 0.8) + 1e-9
+            if nx * ny >= 512 * 512:
+                ideal = ns * (ny + 0.8 * nc) / slots
+                assert waves * (rows + 0.8) <= 1.15 * ideal
+    assert mm.mm_decomposition(2048, 2048, True, 148) == (69, 17, 8)
+    with pytest.raises(mm.MMError):
+        mm.mm_decomposition(0, 5)
+
