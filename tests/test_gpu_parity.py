@@ -211,11 +211,24 @@ def test_smooth14_transmissive(mm, mmo):
     assert_parity(Ug, Uo)
 
 
-@pytest.mark.parametrize("nx,ny", [(1, 1), (3, 2), (5, 1), (33, 9)])
+@pytest.mark.parametrize("nx,ny", [(1, 1), (3, 2), (5, 1), (33, 9), (30, 7), (31, 5), (60, 3), (61, 40)])
 def test_tiny_grids(mm, mmo, nx, ny):
+    """Degenerate and edge sizes: single cells, nx below / at / just above one and two 30-cell strips."""
     prob = wl.random_smooth14(nx, ny, Kn=0.3)
     Ug, Uo = run_both(mm, mmo, prob, 10)
     assert_parity(Ug, Uo)
+
+
+@pytest.mark.parametrize("zsym", [False, True])
+def test_anisotropic_cells_and_mixed_boundaries(mm, mmo, zsym):
+    """dx != dy (dt/dx and dt/dy differ) with periodic x and transmissive y."""
+    prob = wl.random_smooth14(50, 23, Kn=0.1, zsym=zsym, shared_limiter=1)
+    prob = dict(prob, extent=(0.0, 1.0, 0.0, 0.37),
+                bcs=[dict(type=wl.BC_PERIODIC), dict(type=wl.BC_PERIODIC),
+                     dict(type=wl.BC_TRANSMISSIVE), dict(type=wl.BC_TRANSMISSIVE)])
+    dt = 0.5 * scout_dt(mmo, prob, 20, 0.4)
+    Ug, Uo = run_both(mm, mmo, prob, 20, dt=dt)
+    assert_parity(Ug, Uo, max(TOL, 10.0 * roundoff_sensitivity(mmo, prob, 20, dt)))
 
 
 @pytest.mark.parametrize("limiter,flux", [(wl.LIM_MINMOD, wl.FLUX_HLL), (wl.LIM_VANALBADA, wl.FLUX_RUSANOV)])
