@@ -23,7 +23,8 @@ constexpr int kRateNT = 256;
 // 11 x 184 1.46 ms; 12 x 168 1.47 ms -- the closure has enough independent work per thread that
 // registers buy more than extra warps.  Shared memory (strip buffers + the 9 KB a/b table per
 // block) allows 8 (z-symmetric) / 6 (general).
-constexpr size_t kSmemGen = ((size_t)kStripWPB * Mom<false>::warp_smem_doubles + AbTable::kDoubles) * sizeof(double);
+constexpr size_t kSmemGen = ((size_t)kStripWPB * Mom<false>::warp_smem_doubles
+                             + (Mom<false>::table_in_smem ? AbTable::kDoubles : 0)) * sizeof(double);
 constexpr size_t kSmemZS = ((size_t)kStripWPB * Mom<true>::warp_smem_doubles + AbTable::kDoubles) * sizeof(double);
 constexpr int kBlocksByRegs = 8 / kStripWPB;
 constexpr int kBlocksGenSmem = (int)((227 * 1024) / (kSmemGen + 1024));

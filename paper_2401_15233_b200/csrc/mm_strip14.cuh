@@ -50,6 +50,9 @@ struct Mom {
     }
     __host__ __device__ static constexpr int cswap(int k) { return compact(swap_xy(full(k))); }
     static constexpr int warp_smem_doubles = 3 * NV * kRW + 2 * NV * kRW + 2 * NV * 32;
+    // The general variant's strip buffers are 26 KB per warp: with the 9 KB table beside them only 6
+    // warps fit an SM, without it 8.  It reads the table from global memory through L1 instead.
+    static constexpr bool table_in_smem = ZS;
 };
 
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
@@ -78,11 +81,13 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* Uout, Ct
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // the block's copy of the a(P*), b(P*) table (Eq 29c-d), behind the warps' buffers
-    double* tab = smem + kStripWPB * M::warp_smem_doubles;
-    for (int i = threadIdx.x; i < AbTable::kDoubles; i += 32 * kStripWPB) tab[i] = pg.ab[i];
-    __syncthreads();
     Params p = pg;
-    p.ab = tab;
+    if constexpr (M::table_in_smem) {
+        double* tab = smem + kStripWPB * M::warp_smem_doubles;
+        for (int i = threadIdx.x; i < AbTable::kDoubles; i += 32 * kStripWPB) tab[i] = pg.ab[i];
+        __syncthreads();
+        p.ab = tab;
+    }
     const int item = blockIdx.x * kStripWPB + warp;
     if (item >= nstrips * nchunks) return;
     const int strip = item % nstrips, chunk = item / nstrips;
