@@ -21,8 +21,8 @@ constexpr int kRateNT = 256;
 // for: 8, which leaves each thread the full 255 registers (8 x 32 x 256 = the register file).
 // Measured on B200 (2048^2 z-symmetric step): 8 warps x 255 registers 1.30 ms; 10 x 200 1.36 ms;
 // 11 x 184 1.46 ms; 12 x 168 1.47 ms -- the closure has enough independent work per thread that
-// registers buy more than extra warps.  Shared memory (strip buffers + the 9 KB a/b table per
-// block) allows 8 (z-symmetric) / 6 (general).
+// registers buy more than extra warps.  Shared memory allows 8 for both: strip buffers + the 9 KB
+// a/b table per block (z-symmetric), strip buffers alone (general, table through L1).
 constexpr size_t kSmemGen = ((size_t)kStripWPB * Mom<false>::warp_smem_doubles
                              + (Mom<false>::table_in_smem ? AbTable::kDoubles : 0)) * sizeof(double);
 constexpr size_t kSmemZS = ((size_t)kStripWPB * Mom<true>::warp_smem_doubles + AbTable::kDoubles) * sizeof(double);
