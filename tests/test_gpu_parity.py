@@ -362,6 +362,34 @@ def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn):
                 assert np.abs(got[m] - ref[m]).max() <= TOL * scale[m], (ci, cj, m)
 
 
+def test_crossing_jets_reseparate_only_when_collisionless(mm):
+    """The paper's central 2-D result (Fig 13; L472-494, Fig 15; App C): two
+    collisionless jets crossing at a right angle pass through each other and leave the domain
+    straight ahead, which no Euler-like model can do; with many collisions (Kn = 0.01) they merge
+    into one stream leaving along the diagonal.  300^2 cells to t = 0.3 (25 000 and 110 000 steps)."""
+    n = 300
+    yc = (np.arange(n) + 0.5) / n
+    k9, k5 = int(0.9 * n), n // 2
+    out = {}
+    for Kn in (None, 0.01):
+        s = mm.Solver.from_problem(wl.paper_jets(n, two=True, Kn=Kn))
+        s.advance_to(0.3, 0.5)
+        U = s.get_state()
+        assert s.info()["t"] == 0.3 and np.all(np.isfinite(U)) and U[0].min() > 0
+        out[Kn] = U[0]
+    free, coll = out[None], out[0.01]
+    # collisionless: each jet exits opposite to where it entered; nothing leaves through the corner
+    assert abs(yc[free[:, -1].argmax()] - 0.5) < 0.08 and abs(yc[free[-1, :].argmax()] - 0.5) < 0.08
+    assert free[k5, k9] > 5.0 * free[k9, k9] and free[k9, k5] > 5.0 * free[k9, k9]
+    # collisional: one merged stream along the diagonal
+    assert yc[coll[:, -1].argmax()] > 0.65 and yc[coll[-1, :].argmax()] > 0.65
+    assert coll[k9, k9] > coll[k5, k9] and coll[k9, k9] > coll[k9, k5]
+    # the set-up is symmetric under x <-> y and so are both solutions, up to the round-off the scheme
+    # amplifies over 10^4 - 10^5 steps (DESIGN.md R24; the two directions are not evaluated in the same order)
+    for rho in (free, coll):
+        assert np.abs(rho - rho.T).mean() < 0.05 * rho.mean()
+
+
 # ----------------- SURVEY 8(f) items 2-3: midpoint time marching (L250), point-implicit source (L348)
 @pytest.mark.parametrize("opts", [dict(source_scheme=wl.SRC_POINT_IMPLICIT), dict(time_scheme=wl.TIME_MIDPOINT)])
 @pytest.mark.parametrize("case", ["smooth14", "smooth14_zsym", "smooth5", "jets", "sod14"])
