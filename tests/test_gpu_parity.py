@@ -362,6 +362,31 @@ def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn):
                 assert np.abs(got[m] - ref[m]).max() <= TOL * scale[m], (ci, cj, m)
 
 
+def test_single_jet_fast_wave_runs_ahead_of_the_density_front(mm):
+    """PAPER.md L440 (Fig 11): the density front of the collisionless M = 5 jet travels roughly at the
+    jet velocity, waves in the fourth-order moment R* travel "roughly twice as fast", and the gas
+    they have not reached is still at equilibrium with R* = 15 and q* = 0."""
+    n = 300
+    s = mm.Solver.from_problem(wl.paper_jets(n, two=False))
+    xc = (np.arange(n) + 0.5) / n
+    speed_jet = 5.0 * np.sqrt(5.0 / 3.0)
+    fronts = []
+    for t in (0.02, 0.04):
+        s.advance_to(t, 0.5)
+        W = s.get_state_prim()[:, n // 2]                       # the jet axis y = 0.5
+        rho, P = W[0], (W[4] + W[7] + W[9]) / 3.0
+        Rs = W[13] * rho / P ** 2
+        qs = W[10] / (rho * (P / rho) ** 1.5)
+        x_rho = xc[np.nonzero(rho > 0.1)[0].max()]
+        x_R = xc[np.nonzero(np.abs(Rs - 15.0) > 0.15)[0].max()]
+        fronts.append((x_rho, x_R))
+        assert np.allclose(Rs[-10:], 15.0, rtol=1e-12) and np.abs(qs[-10:]).max() < 1e-12
+    v_rho = (fronts[1][0] - fronts[0][0]) / 0.02
+    v_R = (fronts[1][1] - fronts[0][1]) / 0.02
+    assert 0.9 * speed_jet < v_rho < 1.4 * speed_jet            # 6.45: measured 7.7 (front = jet + thermal spread)
+    assert 1.6 < v_R / v_rho < 2.3                              # measured 1.8
+
+
 def test_crossing_jets_reseparate_only_when_collisionless(mm):
     """The paper's central 2-D result (Fig 13; L472-494, Fig 15; App C): two
     collisionless jets crossing at a right angle pass through each other and leave the domain
