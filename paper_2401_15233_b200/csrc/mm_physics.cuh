@@ -54,12 +54,14 @@ __host__ __device__ __forceinline__ void zadd(double&, zero_t) {}
 #ifdef MM_OPCOUNT_HOST
 __forceinline__ double rcp(double x) { return 1.0 / x; }
 __forceinline__ double fsqrt(double x) { return sqrt(x); }
+__forceinline__ double fsqrt_pos(double x) { return sqrt(x); }
 __forceinline__ double rsqrt_nr(double x) { return 1.0 / sqrt(x); }
 __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
 __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 #elif defined(MM_EXACT_MATH)
 __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
 __device__ __forceinline__ double fsqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ double fsqrt_pos(double x) { return sqrt(x); }
 __device__ __forceinline__ double rsqrt_nr(double x) { return 1.0 / sqrt(x); }
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
 __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
@@ -82,6 +84,15 @@ __device__ __forceinline__ double rcp(double x)
     const double e2 = fma(e, e, e);            // e + e^2
     const double e3 = fma(e2, e, e);           // e + e^2 + e^3
     return fma(r, e3, r);                      // r (1 + e + e^2 + e^3): error e^4
+}
+// sqrt(x) for x known to be positive and normal (P/rho, B >= 1): no zero / subnormal guard
+__device__ __forceinline__ double fsqrt_pos(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double s0 = x * y;
+    const double e = fma(-s0, y, 1.0);
+    return fma(s0 * e, fma(0.375, e, 0.5), s0);
 }
 __device__ __forceinline__ double fsqrt(double x)
 {
@@ -269,10 +280,11 @@ __device__ __forceinline__ double inv_tau(const Params& p, double rho, double Ph
 }
 
 // HLL (L256-258; speeds combined as in DESIGN.md R12) or Rusanov (L258) interface flux.
-__device__ __forceinline__ double hll1(double SL, double SR, double SLR, double inv, double FL,
-                                       double FR, double UL, double UR)
+// cL = SR inv, cR = -SL inv, cU = SL SR inv with inv = 1/(SR - SL)
+__device__ __forceinline__ double hll1(double cL, double cR, double cU, double FL, double FR,
+                                       double UL, double UR)
 {
-    return (SR * FL - SL * FR + SLR * (UR - UL)) * inv;
+    return cL * FL + (cR * FR + cU * (UR - UL));
 }
 template <int NM>
 __device__ __forceinline__ void numflux(int flux, const double (&FL)[NM], const double (&FR)[NM],
@@ -287,9 +299,9 @@ __device__ __forceinline__ void numflux(int flux, const double (&FL)[NM], const 
         return;
     }
     double SL = fmin(fmin(lminL, lminR), 0.0), SR = fmax(fmax(lmaxL, lmaxR), 0.0);
-    double inv = rcp(SR - SL), SLR = SL * SR;
+    const double inv = rcp(SR - SL), cL = SR * inv, cR = -SL * inv, cU = SL * cL;
 #pragma unroll
-    for (int m = 0; m < NM; ++m) Fh[m] = hll1(SL, SR, SLR, inv, FL[m], FR[m], UL[m], UR[m]);
+    for (int m = 0; m < NM; ++m) Fh[m] = hll1(cL, cR, cU, FL[m], FR[m], UL[m], UR[m]);
 }
 
 // =========================================================================== 14-moment
@@ -367,7 +379,7 @@ __device__ __forceinline__ void nondim_sigma14(const double (&W)[14], Star14<Z>&
     const double rho = W[0];
     const double Ph = (W[4] + W[7] + W[9]) * (1.0 / 3.0);
     const double rr = rcp(Ph * rho), iP = rr * rho, ir = rr * Ph;      // one reciprocal for both
-    const double c2 = Ph * ir, c = fsqrt(c2);
+    const double c2 = Ph * ir, c = fsqrt_pos(c2);
     s.c = c; s.Ph = Ph;
     s.pxx = W[4] * iP; s.pxy = W[5] * iP; s.pxz = zget<Z>(W[6]) * iP;
     s.pyy = W[7] * iP; s.pyz = zget<Z>(W[8]) * iP; s.pzz = W[9] * iP;
@@ -418,7 +430,7 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
     const double y = rsqrt_nr(sb);                     // sb >= sigma_lim > 0
     t.sb = sb; t.ss = sb * y; t.isb = y * y;
     t.B = 5.0 - 4.0 * t.ss + fsqrt(dmax(10.0 - 16.0 * t.ss + 6.0 * sb, 0.0));   // Eq 29e
-    t.sqB = fsqrt(t.B);
+    t.sqB = fsqrt_pos(t.B);
     return t;
 }
 

@@ -235,11 +235,11 @@ k_step14_strip(const Params pg, const double* __restrict__ Uin, double* Uout, Ct
                     }
                 } else {
                     const double SL = dmin(dmin(lminL, lminR), 0.0), SR = dmax(dmax(lmaxL, lmaxR), 0.0);
-                    const double inv = rcp(SR - SL), SLR = SL * SR;
+                    const double inv = rcp(SR - SL), cL = SR * inv, cR = -SL * inv, cU = SL * cL;
 #pragma unroll
                     for (int k = 0; k < NV; ++k) {
                         const int m = M::full(k);
-                        Fh[k] = hll1(SL, SR, SLR, inv, FL[m], FR[m], UL[m], UR[m]);
+                        Fh[k] = hll1(cL, cR, cU, FL[m], FR[m], UL[m], UR[m]);
                     }
                 }
             }

@@ -86,10 +86,10 @@ static void interface(const Params& p, const cnt (&Wm)[NM], const cnt (&hm)[NM],
     if constexpr (NM == 5) { eval_face5(p, WL, FL, UL, a, b); eval_face5(p, WR, FR, UR, c, d); }
     else { eval_face14<Z>(p, WL, FL, UL, a, b); eval_face14<Z>(p, WR, FR, UR, c, d); }
     const cnt SL = fmin(fmin(a, c), 0.0), SR = fmax(fmax(b, d), 0.0);
-    const cnt inv = rcp(SR - SL), SLR = SL * SR;
+    const cnt inv = rcp(SR - SL), cL = SR * inv, cR = -SL * inv, cU = SL * cL;
     for (int k = 0; k < NM; ++k) {
         if (NM == 14 && zs && z_odd(k)) continue;
-        Fh[k] = hll1(SL, SR, SLR, inv, FL[k], FR[k], UL[k], UR[k]);
+        Fh[k] = hll1(cL, cR, cU, FL[k], FR[k], UL[k], UR[k]);
     }
 }
 
