@@ -108,6 +108,15 @@ __device__ __forceinline__ double fsqrt(double x)
 }
 #endif
 
+// Added to (or used as the floor of) square-root arguments that may be exactly zero or subnormal, so
+// that the guard-free fsqrt_pos applies: sqrt(1e-300) = 1e-150 instead of 0 is far below round-off of
+// the O(1) dimensionless quantities involved; negative / NaN arguments still give NaN.
+#ifdef MM_OPCOUNT_HOST
+static const double kTiny = 1e-300;
+#else
+constexpr double kTiny = 1e-300;
+#endif
+
 // x <-> y swap of the 14 moments (primitive or conserved); an involution.
 __host__ __device__ constexpr int swap_xy(int m)
 {
@@ -193,7 +202,7 @@ __device__ __forceinline__ void prim2cons5(const double (&W)[5], double (&U)[5])
 __device__ __forceinline__ double sigma5(double qs, double rs)
 {
     double b = 3.0 - rs, X = qs * qs;
-    double D = fsqrt(b * b + 8.0 * X);
+    double D = fsqrt_pos(b * b + 8.0 * X + kTiny);
     return b >= 0.0 ? 0.25 * (b + D) : 2.0 * X * rcp(D - b);
 }
 
@@ -202,19 +211,19 @@ struct WS5 { double E, C, Y4, inv2s; };
 __device__ __forceinline__ WS5 ws5_common(double sb)
 {
     WS5 w;
-    double ss = fsqrt(sb);
-    w.C = fsqrt(3.0 - 3.0 * sb);
+    double ss = fsqrt_pos(sb);
+    w.C = fsqrt_pos(3.0 - 3.0 * sb + kTiny);
     w.E = 0.8 * w.C;
-    double B = 5.0 - 4.0 * ss + fsqrt(dmax(10.0 - 16.0 * ss + 6.0 * sb, 0.0));
-    double Y = B + w.E * w.E - 2.0 * w.E * fsqrt(B);
+    double B = 5.0 - 4.0 * ss + fsqrt_pos(dmax(10.0 - 16.0 * ss + 6.0 * sb, kTiny));
+    double Y = B + w.E * w.E - 2.0 * w.E * fsqrt_pos(B);
     w.Y4 = 4.0 * sb * sb * Y;
     w.inv2s = 0.5 * rcp(sb);
     return w;
 }
 __device__ __forceinline__ double ws5_lambda(const WS5& w, double sb, double qs)
 {
-    double rad = dmax(qs * qs - 0.8 * qs * sb * w.C + w.Y4, 0.0);
-    return (qs + fsqrt(rad)) * w.inv2s + w.E;
+    double rad = dmax(qs * qs - 0.8 * qs * sb * w.C + w.Y4, kTiny);
+    return (qs + fsqrt_pos(rad)) * w.inv2s + w.E;
 }
 
 // min / max wave speed of a 5-moment state (Eqs 30, 31, 34).  ok = rho > 0 && P > 0.
@@ -222,7 +231,7 @@ __device__ __forceinline__ void wavespeed5(const Params& p, const double (&W)[5]
                                            double& lmax)
 {
     double rho = W[0], u = W[1], P = W[2], q = W[3], r = W[4];
-    double c2 = P * rcp(rho), c = fsqrt(c2);
+    double c2 = P * rcp(rho), c = fsqrt_pos(c2);
     double irc4 = rcp(rho * c2 * c2);                     // 1/(rho c^4); 1/(rho c^3) = c/(rho c^4)
     double qs = q * (c * irc4), rs = r * irc4;
     double sb = clamp_sigma(sigma5(qs, rs), p.sigma_lim);
@@ -236,13 +245,13 @@ __device__ __forceinline__ void eval_face5(const Params& p, const double (&W)[5]
                                            double (&U)[5], double& lmin, double& lmax)
 {
     double rho = W[0], u = W[1], P = W[2], q = W[3], r = W[4];
-    double c2 = P * rcp(rho), c = fsqrt(c2);
+    double c2 = P * rcp(rho), c = fsqrt_pos(c2);
     double rc3 = rho * c2 * c;
     double irc4 = rcp(rc3 * c);
     double qs = q * (c * irc4), rs = r * irc4;
     double sb = clamp_sigma(sigma5(qs, rs), p.sigma_lim);
     // Eq 15 (L155): s* = q*^3/sigma^2 + (10 - 8 sqrt(sigma)) q*;  s = rho c^5 s*
-    double s = rc3 * c2 * (qs * qs * qs * rcp(sb * sb) + (10.0 - 8.0 * fsqrt(sb)) * qs);
+    double s = rc3 * c2 * (qs * qs * qs * rcp(sb * sb) + (10.0 - 8.0 * fsqrt_pos(sb)) * qs);
     prim2cons5(W, U);
     F[0] = U[1];
     F[1] = U[2];
@@ -275,7 +284,7 @@ __device__ __forceinline__ bool cell_speed5(const Params& p, const double (&W)[5
 __device__ __forceinline__ double inv_tau(const Params& p, double rho, double Ph)
 {
     if (p.tau_model == 1) return p.inv_tau_const;
-    if (p.tau_model == 2) return p.inv_tau_coef * rho * fsqrt(8.0 * Ph * rcp(3.14159265358979323846 * rho));
+    if (p.tau_model == 2) return p.inv_tau_coef * rho * fsqrt_pos(8.0 * Ph * rcp(3.14159265358979323846 * rho));
     return 0.0;
 }
 
@@ -417,7 +426,7 @@ __device__ __forceinline__ void nondim_sigma14(const double (&W)[14], Star14<Z>&
     // Eq 21 with P_ii P_jj = 9: sigma = [b + sqrt(b^2 + 8 t2 X)]/(4 t2), b = 2 t2 + 9 - R*,
     // X = h.p^-1.h; conjugate form when b < 0 (R4)
     const double b = 2.0 * s.t2 + 9.0 - Rs;
-    const double D = fsqrt(b * b + 8.0 * s.t2 * X);
+    const double D = fsqrt_pos(b * b + 8.0 * s.t2 * X + kTiny);       // kTiny: no zero / subnormal argument
     const bool pos = b >= 0.0;
     s.sigma = (pos ? b + D : 2.0 * X) * rcp(pos ? 4.0 * s.t2 : D - b);
 }
@@ -429,7 +438,7 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
     SbTerms t;
     const double y = rsqrt_nr(sb);                     // sb >= sigma_lim > 0
     t.sb = sb; t.ss = sb * y; t.isb = y * y;
-    t.B = 5.0 - 4.0 * t.ss + fsqrt(dmax(10.0 - 16.0 * t.ss + 6.0 * sb, 0.0));   // Eq 29e
+    t.B = 5.0 - 4.0 * t.ss + fsqrt_pos(dmax(10.0 - 16.0 * t.ss + 6.0 * sb, kTiny));   // Eq 29e
     t.sqB = fsqrt_pos(t.B);
     return t;
 }
@@ -513,7 +522,7 @@ __device__ __forceinline__ void ws14_dir(const double* __restrict__ ab, double P
 {
     double a, b;
     ab_eval(ab, Pdd, a, b);
-    const double C = fsqrt((3.0 - 3.0 * t.sb) * Pdd);
+    const double C = fsqrt_pos((3.0 - 3.0 * t.sb) * Pdd + kTiny);
     const double E = 0.8 * C;
     const double sY = t.sqB - E;
     const double pref = (a * t.sb + b) * (0.5 * t.isb);
@@ -521,9 +530,9 @@ __device__ __forceinline__ void ws14_dir(const double* __restrict__ ab, double P
     const double cst = 4.0 * t.sb * t.sb * (sY * sY) + 0.1 * qt2;
     const double alpha = (0.6 * Pdd - 0.38) * Pdd + 0.35;            // Eq 29b
     const double zp = hd + alpha * qt, zm = -hd + alpha * qt;        // Eq 30: q_d -> -q_d
-    const double rp = dmax(zp * zp - zp * sC + cst, 0.0), rm = dmax(zm * zm - zm * sC + cst, 0.0);
-    lam_max = pref * (zp + fsqrt(rp)) + E;
-    lam_min_neg = pref * (zm + fsqrt(rm)) + E;
+    const double rp = dmax(zp * zp - zp * sC + cst, kTiny), rm = dmax(zm * zm - zm * sC + cst, kTiny);
+    lam_max = pref * (zp + fsqrt_pos(rp)) + E;
+    lam_min_neg = pref * (zm + fsqrt_pos(rm)) + E;
 }
 
 // lambda_min / lambda_max along x of an (index-swapped for y) state, Eqs 28-31 (L388-411).
