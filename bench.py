@@ -53,7 +53,7 @@ def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14):
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None where no capture of that configuration exists).
 NCU_TRAFFIC_BYTES = {
-    ("k_step14_strip<zsym>", 2048): (352.04e6 + 423.10e6, "profiles/r1h_k_step14_strip_zsym.md"),
+    ("k_step14_strip<zsym>", 2048): (351.97e6 + 423.15e6, "profiles/r1m_k_step14_strip_zsym.md"),
 }
 
 
