@@ -109,12 +109,13 @@ __device__ __forceinline__ double fsqrt(double x)
 #endif
 
 // Added to (or used as the floor of) square-root arguments that may be exactly zero or subnormal, so
-// that the guard-free fsqrt_pos applies: sqrt(1e-300) = 1e-150 instead of 0 is far below round-off of
+// that the guard-free fsqrt_pos applies: sqrt(1.5e-300) = 1.2e-150 instead of 0 is far below round-off of
 // the O(1) dimensionless quantities involved; negative / NaN arguments still give NaN.
+// 2^-996 ~ 1.5e-300: a power of two has a zero low word, so it is an instruction immediate
 #ifdef MM_OPCOUNT_HOST
-static const double kTiny = 1e-300;
+static const double kTiny = 0x1p-996;
 #else
-constexpr double kTiny = 1e-300;
+constexpr double kTiny = 0x1p-996;
 #endif
 
 // x <-> y swap of the 14 moments (primitive or conserved); an involution.
