@@ -307,6 +307,7 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
     p.source_scheme = opt->source_scheme; s->time_scheme = opt->time_scheme;
     p.nx = grid->nx; p.ny = grid->ny; p.pitch = L.pitch; p.rows = L.rows;
     p.ab = (const double*)(s->ws + L.off_tab);
+    p.set_constants();
 
     // boundary tables: copy, and mark which entries some ghost cell actually takes
     BcTable* hb = new (std::nothrow) BcTable();
@@ -667,6 +668,7 @@ int mm_batch5_create(mm_batch5** out, int nx, int ntubes, double x0, double x1, 
     p.ws_scale = ws_scale; p.dx = (x1 - x0) / nx; p.dy = 1.0; p.x0 = x0;
     p.limiter = limiter; p.shared_limiter = shared_limiter ? 1 : 0; p.flux = flux;
     p.nx = nx; p.ny = 1;
+    p.set_constants();
     std::vector<double> itc(ntubes);
     for (int j = 0; j < ntubes; ++j) itc[j] = Kn[j] > 0.0 ? 1.0 / (Kn[j] * L_ref * rho_ref) : 0.0;   // <= 0: collisionless
     cudaError_t e = cudaMemsetAsync(b->ws, 0, L.off_u0, b->stream);

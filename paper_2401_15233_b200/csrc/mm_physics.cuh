@@ -137,6 +137,10 @@ struct Params {               // per-solver constants, passed by value to the ke
     int source_scheme;        // 0 explicit, 1 point-implicit (L348)
     int nx, ny, pitch, rows;  // padded array: rows x pitch doubles per moment, interior at (+2,+2)
     const double* ab;         // table of the functions a(P*), b(P*) of Eq 29c-d (AbTable below)
+    // Literals whose low word is not zero (0.8, 0.1, ... of Eq 29, 1/3) cost two register moves per use
+    // as immediates; as kernel parameters they are constant-bank operands of the FP64 instructions.
+    double k08, k01, k06, k038, k035, k13;
+    __host__ void set_constants() { k08 = 0.8; k01 = 0.1; k06 = 0.6; k038 = 0.38; k035 = 0.35; k13 = 1.0 / 3.0; }
 };
 
 __device__ __forceinline__ double clamp_sigma(double s, double lim)
@@ -517,19 +521,19 @@ __forceinline__ void ab_eval(const double* tab, double P, double& a, double& b)
 // heat flux along (hd) and across (qt2 = sum of squares of the other two), sigma_bar terms.
 // a(P*), b(P*) come from the table (ab_eval); Y = B + E^2 - 2 E sqrt(B)
 // is evaluated as (sqrt(B) - E)^2; the radicand is floored at 0 (R6).
-__device__ __forceinline__ void ws14_dir(const double* __restrict__ ab, double Pdd, double hd,
+__device__ __forceinline__ void ws14_dir(const Params& p, double Pdd, double hd,
                                          double qt, double qt2, const SbTerms& t, double& lam_max,
                                          double& lam_min_neg)
 {
     double a, b;
-    ab_eval(ab, Pdd, a, b);
+    ab_eval(p.ab, Pdd, a, b);
     const double C = fsqrt_pos((3.0 - 3.0 * t.sb) * Pdd + kTiny);
-    const double E = 0.8 * C;
+    const double E = p.k08 * C;
     const double sY = t.sqB - E;
     const double pref = (a * t.sb + b) * (0.5 * t.isb);
-    const double sC = 0.8 * t.sb * C;
-    const double cst = 4.0 * t.sb * t.sb * (sY * sY) + 0.1 * qt2;
-    const double alpha = (0.6 * Pdd - 0.38) * Pdd + 0.35;            // Eq 29b
+    const double sC = t.sb * E;
+    const double cst = 4.0 * t.sb * t.sb * (sY * sY) + p.k01 * qt2;
+    const double alpha = (p.k06 * Pdd - p.k038) * Pdd + p.k035;      // Eq 29b
     const double zp = hd + alpha * qt, zm = -hd + alpha * qt;        // Eq 30: q_d -> -q_d
     const double rp = dmax(zp * zp - zp * sC + cst, kTiny), rm = dmax(zm * zm - zm * sC + cst, kTiny);
     lam_max = pref * (zp + fsqrt_pos(rp)) + E;
@@ -544,7 +548,7 @@ __device__ __forceinline__ void wavespeed14_x(const Params& p, const Star14<Z>& 
     double a, b, qt;                                                 // Eq 28: qtilde >= 0 (R7)
     const double qt2 = s.hy * s.hy + s.hz * s.hz;
     if constexpr (std::is_same<Z, zero_t>::value) qt = fabs(s.hy); else qt = fsqrt(qt2);
-    ws14_dir(p.ab, s.pxx, s.hx, qt, qt2, t, a, b);
+    ws14_dir(p, s.pxx, s.hx, qt, qt2, t, a, b);
     const double kc = p.ws_scale * s.c;
     lmax = ux + kc * a; lmin = ux - kc * b;
 }
@@ -556,7 +560,7 @@ __device__ __forceinline__ void wavespeed14_y(const Params& p, const Star14<Z>& 
     double a, b, qt;
     const double qt2 = s.hx * s.hx + s.hz * s.hz;
     if constexpr (std::is_same<Z, zero_t>::value) qt = fabs(s.hx); else qt = fsqrt(qt2);
-    ws14_dir(p.ab, s.pyy, s.hy, qt, qt2, t, a, b);
+    ws14_dir(p, s.pyy, s.hy, qt, qt2, t, a, b);
     const double kc = p.ws_scale * s.c;
     lmax = uy + kc * a; lmin = uy - kc * b;
 }

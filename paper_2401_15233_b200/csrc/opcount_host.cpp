@@ -140,6 +140,7 @@ int main()
     static cnt dummy_tab[AbTable::kStride];        // coefficients do not matter for the count
     for (auto& c : dummy_tab) c = cnt(0.5);
     p.ab = dummy_tab;
+    p.set_constants();
     p.sigma_lim = 1e-4; p.ws_scale = 1.0; p.dx = 0.01; p.dy = 0.01;
     p.inv_tau_coef = 100.0; p.tau_model = 2; p.limiter = 1; p.flux = 0;
     for (int shared = 0; shared < 2; ++shared) {
