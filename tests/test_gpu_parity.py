@@ -321,8 +321,8 @@ def test_C3_jets_developed_state(mm, mmo):
     assert_parity(sg.get_state(), so.get_state(), max(1e-9, 10.0 * rel_err(sp.get_state(), so.get_state()).max()))
 
 
-@pytest.mark.parametrize("n,Kn", [(2048, 0.1), (2048, 1.0), (4096, 0.1)])
-def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn):
+@pytest.mark.parametrize("n,Kn,fast", [(2048, 0.1, True), (2048, 1.0, True), (4096, 0.1, True), (2048, 0.1, False)])
+def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn, fast):
     """Full bench sizes (BASELINE configs[3] and [4]), bench launch configuration: after n steps a
     cell depends only on the (2n)-neighbourhood of its initial data, so the oracle is run on small
     windows of the same seeded state (transmissive window edges) and compared on the cells no edge
@@ -330,6 +330,8 @@ def test_C4_C5_jets_full_size_sampled_windows(mm, mmo, n, Kn):
     nsteps, half, margin = 3, 14, 2 * 3 + 1
     prob = wl.crossed_jets(n, Kn=Kn, perturb=0.01)
     sg = mm.Solver.from_problem(prob)
+    sg.set_fast_path(fast)                     # z-symmetric variant (what bench.py runs) or the general one
+    assert sg.fast_path_active == fast
     so_dt = 0.5 * 0.4 * (1.0 / n) / 6.0        # CFL 0.2 against the jets' inflow speed (~5.8)
     sg.step_fixed_dt(nsteps, so_dt)
     Ug = sg.get_state()
