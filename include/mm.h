@@ -56,6 +56,14 @@ typedef struct mm_solver mm_solver;   /* opaque, host object; freed by mm_destro
 /* Grid: nx x ny interior cells on [x0,x1] x [y0,y1]; ny = 1 (y0,y1 ignored) for MM_SYS5_1D. */
 typedef struct { int system; int nx, ny; double x0, x1, y0, y1; } mm_grid;
 
+/* Gas (Eq 6; L284): the specific gas constant R in T = P/(rho R).  The moment systems themselves
+ * never see a temperature (the state is rho, u, P, q, R_iijj); R_gas enters where the problem
+ * statement gives one: Dirichlet states given as Maxwellians (rho, u, T) (mm_bc.band_state, L426:
+ * "imposing the said values [rho_jet, u_jet, T_jet] into the ghost cells").  gas == NULL means
+ * R_gas = 1 (the non-dimensional configs of BASELINE.json).  The adiabatic exponent is implied by
+ * the system: 3 for the 1D1V 5-moment gas, 5/3 for the 14-moment gas. */
+typedef struct { double R_gas; } mm_gas;
+
 /* BGK relaxation time (L284, L474):
  *   MM_TAU_NONE  collisionless, source disabled (L432)
  *   MM_TAU_CONST tau
@@ -69,9 +77,14 @@ typedef struct { int model; double tau, Kn, L_ref, rho_ref; } mm_collision;
  *   MM_BC_DIRICHLET    piecewise-constant PRIMITIVE states along the side (inflow jets, L426):
  *                      band k holds where the cell-centre coordinate along the side is in
  *                      [band_lo[k], band_hi[k]]; elsewhere default_W, or zero-gradient when
- *                      default_W == NULL.  nbands <= MM_MAX_BANDS; band_W is [nbands][nmom]. */
+ *                      default_W == NULL.  nbands <= MM_MAX_BANDS.
+ *   band_state         MM_STATE_PRIMITIVE: band_W is [nbands][nmom] and default_W [nmom] primitives W;
+ *                      MM_STATE_MAXWELLIAN: band_W is [nbands][5] and default_W [5] = (rho, u_x, u_y, u_z, T)
+ *                      (u_y, u_z ignored by MM_SYS5_1D), expanded ON THE DEVICE to the Maxwellian of L73 /
+ *                      L127: P_ij = rho R_gas T delta_ij, q = 0, R_iijj = 15 P^2/rho (5-moment r = 3 P^2/rho). */
+enum { MM_STATE_PRIMITIVE = 0, MM_STATE_MAXWELLIAN = 1 };
 typedef struct { int type; int nbands; const double *band_lo, *band_hi, *band_W;
-                 const double *default_W; } mm_bc;
+                 const double *default_W; int band_state; } mm_bc;
 
 typedef struct {
     double sigma_lim;     /* lower limit of sigma inside closure + wave speeds (L163, L512); 1e-4 */
@@ -92,8 +105,10 @@ typedef struct {
  * tables, control block, wave-speed table, dt history).  0 on invalid grid. */
 size_t mm_workspace_bytes(const mm_grid *grid);
 
-/* Build a solver on caller-provided device memory.  d_workspace: DEVICE pointer. */
-int mm_create(mm_solver **out, const mm_grid *grid, const mm_collision *collision,
+/* Build a solver on caller-provided device memory (problem statement of section 3 L250 and section 6
+ * L426: grid, gas, relaxation-time model, boundary data).  d_workspace: DEVICE pointer.  gas may be
+ * NULL (R_gas = 1); MM_EINVAL if R_gas <= 0. */
+int mm_create(mm_solver **out, const mm_grid *grid, const mm_gas *gas, const mm_collision *collision,
               const mm_bc bcs[4], const mm_options *options, void *d_workspace, size_t bytes);
 
 /* Load the interior state (conserved resp. primitive moments, [nmom][ny][nx]), fill the ghost
@@ -149,23 +164,14 @@ long long mm_launch_count(const mm_solver *s);
 int mm_set_fast_path(mm_solver *s, int allow);
 int mm_fast_path_active(const mm_solver *s);
 
-/* Measurement hooks (used by bench.py for the roofline line).
+/* Launch timing (used by bench.py for the roofline line; creates CUDA events, no
+ * device memory).  The hooks that need device scratch of their own (FP64 peak probe, accuracy self-test
+ * of the elementary functions) are NOT part of this library: include/mm_bench.h, libmm_bench.so.
  * Between mm_profile_begin and mm_profile_end every launch of the fused step kernel is
  * bracketed by CUDA events on the solver's stream; mm_profile_end synchronises and returns the
  * summed device time of those launches (milliseconds) and their number. */
 int mm_profile_begin(mm_solver *s);
 int mm_profile_end(mm_solver *s, double *step_kernel_ms, long long *launches);
-/* FP64 FMA peak of the current device, measured with a register-resident DFMA loop on
- * `stream` (cudaStream_t): 2 flop per FMA, best of `repeats` launches.  This is the roofline
- * denominator of this FP64-ALU-bound method; MEASURED_PEAKS.json has no FP64 entry. */
-int mm_measure_fp64_peak(void *stream, int repeats, double *tflops);
-/* Accuracy of the library's own elementary functions, measured on `stream` over n pseudo-random
- * arguments: max relative error in units of 2^-53 of
- * max_ulp[0] the branch-free reciprocal and [1] square root against IEEE (1e-30 .. 1e30),
- * [2] the tabulated a(P*), b(P*) of Eq 29c-d on (0, 3] against the direct formulas with libm
- *     pow / exp (whose own conditioning, P*^2 eps in the exponent, is ~10 units at P* = 3). */
-int mm_selftest_fastmath(void *stream, int n, double max_ulp[3]);
-
 /* ---- Batched 1-D 5-moment solver: `ntubes` independent shock tubes
  * of nx cells on [x0, x1], transmissive ends (L426), each with its own sigma_lim (L163) and Knudsen
  * number (tau = Kn L_ref (rho_ref/rho)/sqrt(8P/(pi rho)), L284; Kn <= 0: collisionless), its own CFL

@@ -115,6 +115,14 @@ double mmo_limiter_psi(int limiter, double dm, double dp);
 /* Limited slope used in per-variable mode: minmod(dm,dp) resp. dm dp (dm+dp)/(dm^2+dp^2). */
 double mmo_limited_slope(int limiter, double dm, double dp);
 
+/* MUSCL face states of one cell along one direction from the primitives of the low neighbour Wm,
+ * the cell W0 and the high neighbour Wp (L262-266): Wlo = W0 - slope/2, Whi = W0 + slope/2 with
+ * slope_k = psi_k (dm_k + dp_k)/2 per variable, or -- shared_limiter (L266) -- one psi = min_k psi_k
+ * for all nm variables, a variable with dm = dp = 0 exactly imposing no constraint (reading R14).
+ * Pinned by hand-computed three-cell examples (tests/test_oracle_scheme.py). */
+void mmo_face_states(int nm, int limiter, int shared_limiter, const double *Wm, const double *W0,
+                     const double *Wp, double *Wlo, double *Whi);
+
 /* HLL (L256-258; reading R12) or Rusanov (L258) interface flux for n components. */
 void mmo_numflux(int flux, int n, const double *FL, const double *FR, const double *UL,
                  const double *UR, double lminL, double lmaxL, double lminR, double lmaxR,

@@ -96,6 +96,7 @@ def bind(L):
         "mmo_tau": (d, [i, d, d, d, d, d, d]),
         "mmo_limiter_psi": (d, [i, d, d]), "mmo_limited_slope": (d, [i, d, d]),
         "mmo_numflux": (None, [i, i, p, p, p, p, d, d, d, d, p]),
+        "mmo_face_states": (None, [i, i, i, p, p, p, p, p]),
         "mmo_create": (i, [C.POINTER(C.c_void_p), C.POINTER(_Grid), C.POINTER(_Collision),
                            C.POINTER(_BC), C.POINTER(_Options)]),
         "mmo_set_state": (i, [C.c_void_p, p]), "mmo_set_state_prim": (i, [C.c_void_p, p]),
@@ -225,6 +226,15 @@ def limiter_psi(limiter, dm, dp):
 
 def limited_slope(limiter, dm, dp):
     return lib().mmo_limited_slope(limiter, dm, dp)
+
+
+def face_states(limiter, shared, Wm, W0, Wp):
+    """MUSCL face states (low, high) of the middle cell (L262-266)."""
+    Wm, W0, Wp = _arr(Wm), _arr(W0), _arr(Wp)
+    n = W0.size
+    lo, hi = np.empty(n), np.empty(n)
+    lib().mmo_face_states(n, limiter, int(shared), _ptr(Wm), _ptr(W0), _ptr(Wp), _ptr(lo), _ptr(hi))
+    return lo, hi
 
 
 def numflux(flux, FL, FR, UL, UR, lminL, lmaxL, lminR, lmaxR):

@@ -336,13 +336,13 @@ static double max_rate(mmo_solver *s, double *max_speed)
 
 /* ---- step 4: limited slopes and face states of cell c along one direction (L262-266).
  * Wm, W0, Wp: primitives of the low neighbour, the cell, the high neighbour.
- * Wlo = W0 - slope/2 (low face), Whi = W0 + slope/2 (high face). */
-static void face_states(const mmo_solver *s, const double *Wm, const double *W0,
-                        const double *Wp, double *Wlo, double *Whi)
+ * Wlo = W0 - slope/2 (low face), Whi = W0 + slope/2 (high face).
+ * Exported so that tests/test_oracle_scheme.py can pin it against hand-computed face values. */
+void mmo_face_states(int nm, int lim, int shared_limiter, const double *Wm, const double *W0,
+                     const double *Wp, double *Wlo, double *Whi)
 {
-    int nm = s->nm, lim = s->opt.limiter;
     double slope[14];
-    if (s->opt.shared_limiter && lim != MMO_LIM_NONE) {
+    if (shared_limiter && lim != MMO_LIM_NONE) {
         /* L266: the same, most stringent limiter value for all primitive variables.
          * A variable with dm = dp = 0 imposes no constraint (reading R14). */
         double psi = 1.0;
@@ -364,6 +364,12 @@ static void face_states(const mmo_solver *s, const double *Wm, const double *W0,
         Wlo[k] = W0[k] - 0.5 * slope[k];
         Whi[k] = W0[k] + 0.5 * slope[k];
     }
+}
+
+static void face_states(const mmo_solver *s, const double *Wm, const double *W0,
+                        const double *Wp, double *Wlo, double *Whi)
+{
+    mmo_face_states(s->nm, s->opt.limiter, s->opt.shared_limiter, Wm, W0, Wp, Wlo, Whi);
 }
 
 /* ---- step 5: interface flux between cell a (low side) and cell b (high side) along d.

@@ -8,9 +8,12 @@ from pathlib import Path
 
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
-LIB = PKG / "libmm.so"
+LIB = PKG / "libmm.so"                 # the product: include/mm.h
+BENCH_LIB = PKG / "libmm_bench.so"     # measurement / self-test hooks: include/mm_bench.h (allocates its own scratch)
 SOURCES = ["mm_api.cu"]
+BENCH_SOURCES = ["mm_bench.cu"]
 DEPS = ["mm_api.cu", "mm_kernels.cuh", "mm_strip14.cuh", "mm_batch5.cuh", "mm_physics.cuh", "../../include/mm.h"]
+BENCH_DEPS = ["mm_bench.cu", "mm_kernels.cuh", "mm_physics.cuh", "../../include/mm_bench.h"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]
 
@@ -22,26 +25,39 @@ def nvcc_path() -> str:
     raise RuntimeError("nvcc not found: the CUDA library cannot be built (there is no CPU fallback)")
 
 
-def stale() -> bool:
-    if not LIB.exists():
+def stale(lib: Path = LIB, deps=None) -> bool:
+    if not lib.exists():
         return True
-    t = LIB.stat().st_mtime
-    return any((CSRC / d).resolve().stat().st_mtime > t for d in DEPS)
+    t = lib.stat().st_mtime
+    return any((CSRC / d).resolve().stat().st_mtime > t for d in (deps or DEPS))
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not stale():
-        return LIB
+def _compile(lib: Path, sources, verbose: bool) -> Path:
     cmd = [nvcc_path(), *NVCC_FLAGS]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += ["-o", str(LIB), *[str(CSRC / s) for s in SOURCES]]
+    cmd += ["-o", str(lib), *[str(CSRC / s) for s in sources]]
     subprocess.run(cmd, check=True, cwd=CSRC)
-    return LIB
+    return lib
+
+
+def build(force: bool = False, verbose: bool = False) -> Path:
+    """libmm.so, the product library."""
+    if not force and not stale():
+        return LIB
+    return _compile(LIB, SOURCES, verbose)
+
+
+def build_bench(force: bool = False, verbose: bool = False) -> Path:
+    """libmm_bench.so, the measurement hooks of include/mm_bench.h."""
+    if not force and not stale(BENCH_LIB, BENCH_DEPS):
+        return BENCH_LIB
+    return _compile(BENCH_LIB, BENCH_SOURCES, verbose)
 
 
 if __name__ == "__main__":
     print(build(force=True, verbose=True))
+    print(build_bench(force=True, verbose=True))
 
 
 OPCOUNT_TXT = PKG / "opcount.txt"

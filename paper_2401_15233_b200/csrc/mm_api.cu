@@ -94,6 +94,7 @@ struct mm_solver {
     int cur;            // buffer holding the current state
     int slot;           // accumulator slot holding the current state's CFL reduction
     int has_state;
+    long long hist_first;   // dt history is valid for steps >= hist_first (mm_set_clock moves it)
     long long launches;
     int nstrips, nchunks[2];   // 14-moment work decomposition (mm_strip14.cuh): [general, z-symmetric]
     int time_scheme;        // MM_TIME_EULER | MM_TIME_MIDPOINT
@@ -207,7 +208,7 @@ int set_state_impl(mm_solver* s, const double* src, int on_device, bool prim)
         MM_CUDA(cudaMemcpyAsync(s->U[s->cur ^ 1], src, nbytes, cudaMemcpyHostToDevice, s->stream));
         dsrc = s->U[s->cur ^ 1];
     }
-    dim3 grid((s->p.nx + 127) / 128, s->p.ny);
+    dim3 grid((s->p.nx + 127) / 128, s->p.ny < 65535 ? s->p.ny : 65535);
     if (prim) k_pack<NM, true><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur]);
     else k_pack<NM, false><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur]);
     MM_LAUNCHED(s, "k_pack");
@@ -215,6 +216,7 @@ int set_state_impl(mm_solver* s, const double* src, int on_device, bool prim)
     MM_CUDA(cudaMemsetAsync(s->ctrl, 0, offsetof(Ctrl, ghost_rate), s->stream));
     MM_CUDA(cudaMemsetAsync(&s->ctrl->steps, 0, sizeof(Ctrl) - offsetof(Ctrl, steps), s->stream));
     s->slot = 0;
+    s->hist_first = 0;
     StepCtl none = {0, 0.0, -1.0};
     int rc = launch_ghost<NM>(s, none, 0);
     if (rc) return rc;
@@ -237,7 +239,7 @@ int get_state_impl(mm_solver* s, double* dst, int on_device, bool prim)
 {
     const size_t nbytes = (size_t)NM * s->p.nx * s->p.ny * sizeof(double);
     double* ddst = on_device ? dst : s->U[s->cur ^ 1];
-    dim3 grid((s->p.nx + 127) / 128, s->p.ny);
+    dim3 grid((s->p.nx + 127) / 128, s->p.ny < 65535 ? s->p.ny : 65535);
     if (prim) k_unpack<NM, true><<<grid, 128, 0, s->stream>>>(s->p, s->U[s->cur], ddst);
     else k_unpack<NM, false><<<grid, 128, 0, s->stream>>>(s->p, s->U[s->cur], ddst);
     MM_LAUNCHED(s, "k_unpack");
@@ -257,10 +259,11 @@ size_t mm_workspace_bytes(const mm_grid* grid)
     return make_layout(grid, &L) ? L.total : 0;
 }
 
-int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, const mm_bc bcs[4],
-              const mm_options* opt, void* d_workspace, size_t bytes)
+int mm_create(mm_solver** out, const mm_grid* grid, const mm_gas* gas, const mm_collision* col,
+              const mm_bc bcs[4], const mm_options* opt, void* d_workspace, size_t bytes)
 {
     if (!out || !grid || !col || !bcs || !opt) return MM_EINVAL;
+    if (gas && !(gas->R_gas > 0.0)) return MM_EINVAL;
     Layout L;
     if (!make_layout(grid, &L)) return MM_EINVAL;
     if (!(opt->sigma_lim > 0.0) || !(opt->ws_scale > 0.0)) return MM_EINVAL;
@@ -276,6 +279,7 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
         if (bcs[b].type == MM_BC_DIRICHLET) {
             if (bcs[b].nbands < 0 || bcs[b].nbands > MM_MAX_BANDS) return MM_EINVAL;
             if (bcs[b].nbands > 0 && (!bcs[b].band_lo || !bcs[b].band_hi || !bcs[b].band_W)) return MM_EINVAL;
+            if (bcs[b].band_state != MM_STATE_PRIMITIVE && bcs[b].band_state != MM_STATE_MAXWELLIAN) return MM_EINVAL;
         }
     }
     for (int d = 0; d < ndim; ++d)
@@ -302,6 +306,7 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
     p.x0 = grid->x0; p.y0 = ndim == 2 ? grid->y0 : 0.0;
     p.inv_tau_coef = col->model == MM_TAU_KN ? 1.0 / (col->Kn * col->L_ref * col->rho_ref) : 0.0;
     p.inv_tau_const = col->model == MM_TAU_CONST ? 1.0 / col->tau : 0.0;
+    p.R_gas = gas ? gas->R_gas : 1.0;
     p.tau_model = col->model; p.limiter = opt->limiter;
     p.shared_limiter = opt->shared_limiter ? 1 : 0; p.flux = opt->flux;
     p.source_scheme = opt->source_scheme; s->time_scheme = opt->time_scheme;
@@ -320,11 +325,13 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_collision* col, con
         if (sd.type != MM_BC_DIRICHLET) continue;
         sd.nbands = bcs[b].nbands;
         sd.has_default = bcs[b].default_W ? 1 : 0;
+        sd.maxwellian = bcs[b].band_state == MM_STATE_MAXWELLIAN;
+        const int nw = sd.maxwellian ? 5 : nm;         // doubles per state as given (expanded by k_bc_table)
         for (int k = 0; k < sd.nbands; ++k) {
             sd.lo[k] = bcs[b].band_lo[k]; sd.hi[k] = bcs[b].band_hi[k];
-            memcpy(sd.W[k], bcs[b].band_W + (size_t)k * nm, nm * sizeof(double));
+            memcpy(sd.W[k], bcs[b].band_W + (size_t)k * nw, nw * sizeof(double));
         }
-        if (sd.has_default) memcpy(sd.W[sd.nbands], bcs[b].default_W, nm * sizeof(double));
+        if (sd.has_default) memcpy(sd.W[sd.nbands], bcs[b].default_W, nw * sizeof(double));
         const int n = b < 2 ? grid->ny : grid->nx;
         for (int pos = 0; pos < n; ++pos) {
             const double coord = b < 2 ? p.y0 + ((double)pos + 0.5) * p.dy : p.x0 + ((double)pos + 0.5) * p.dx;
@@ -470,6 +477,7 @@ int mm_get_dt_history(mm_solver* s, long long first_step, int n, double* dt)
     Ctrl h;
     int rc = read_ctrl(s, &h);
     if (rc) return rc;
+    if (first_step < s->hist_first) return MM_EINVAL;                                      // before this solver's own steps
     if (first_step + n > h.steps || h.steps - first_step > kDtHistory) return MM_EINVAL;   // not taken yet / overwritten
     const double* hist = (const double*)(s->ws + s->L.off_hist);
     for (int k = 0; k < n;) {                      // the ring wraps at most once inside the range
@@ -488,6 +496,7 @@ int mm_set_clock(mm_solver* s, double t, long long steps)
     MM_CUDA(cudaMemcpyAsync(&s->ctrl->t, &t, sizeof t, cudaMemcpyHostToDevice, s->stream));
     MM_CUDA(cudaMemcpyAsync(&s->ctrl->steps, &steps, sizeof steps, cudaMemcpyHostToDevice, s->stream));
     MM_CUDA(cudaStreamSynchronize(s->stream));     // t and steps are stack variables
+    s->hist_first = steps;                         // steps before the restored counter were not taken here
     return MM_OK;
 }
 
@@ -535,56 +544,6 @@ int mm_profile_end(mm_solver* s, double* step_kernel_ms, long long* launches)
     if (launches) *launches = (long long)(s->ev.size() / 2);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     s->ev.clear();
-    return MM_OK;
-}
-
-int mm_measure_fp64_peak(void* stream, int repeats, double* tflops)
-{
-    if (!tflops || repeats < 1) return MM_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    int dev = 0, sms = 0;
-    MM_CUDA(cudaGetDevice(&dev));
-    MM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    double* d_out = nullptr;
-    MM_CUDA(cudaMalloc(&d_out, sizeof(double)));      // measurement scratch only, not solver memory
-    cudaEvent_t e0, e1;
-    MM_CUDA(cudaEventCreate(&e0));
-    MM_CUDA(cudaEventCreate(&e1));
-    const int iters = 20000, blocks = sms * 8, threads = 256;
-    double best = 0.0;
-    for (int r = 0; r < repeats + 1; ++r) {            // first launch is the warm-up
-        cudaEventRecord(e0, st);
-        k_dfma_peak<<<blocks, threads, 0, st>>>(d_out, iters, 0.999999, 1e-6);
-        cudaEventRecord(e1, st);
-        cudaError_t e = cudaEventSynchronize(e1);
-        if (e != cudaSuccess) { cudaFree(d_out); return cuda_fail(e, "k_dfma_peak"); }
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        double tf = 2.0 * 16.0 * (double)iters * blocks * threads / (ms * 1e-3) * 1e-12;
-        if (r > 0 && tf > best) best = tf;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
-    *tflops = best;
-    return MM_OK;
-}
-
-int mm_selftest_fastmath(void* stream, int n, double* max_ulp)
-{
-    if (n < 1 || !max_ulp) return MM_EINVAL;
-    double* tab = nullptr;
-    cudaStream_t st = (cudaStream_t)stream;
-    unsigned long long* d = nullptr;
-    MM_CUDA(cudaMalloc(&d, 8 * sizeof(unsigned long long)));   // measurement scratch only
-    MM_CUDA(cudaMalloc(&tab, AbTable::kDoubles * sizeof(double)));
-    cudaMemsetAsync(d, 0, 8 * sizeof(unsigned long long), st);
-    k_ab_table<<<AbTable::kIntervals, 2, 0, st>>>(tab);
-    k_fastmath_test<<<296, 256, 0, st>>>(n, d, tab);
-    unsigned long long h[3] = {0, 0, 0};
-    cudaError_t e = cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(d); cudaFree(tab);
-    if (e != cudaSuccess) return cuda_fail(e, "k_fastmath_test");
-    for (int k = 0; k < 3; ++k) max_ulp[k] = bits2d(h[k]);
     return MM_OK;
 }
 

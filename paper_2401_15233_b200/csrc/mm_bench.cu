@@ -1,0 +1,127 @@
+// mm_bench.cu -- measurement / self-test hooks (include/mm_bench.h), built as libmm_bench.so.
+// Not part of the product library: these allocate a few KB of device scratch of their own.
+#include "../../include/mm_bench.h"
+#include "mm_kernels.cuh"
+
+#include <cstring>
+
+using namespace mm;
+
+namespace {
+
+// Register-resident DFMA loop: 16 independent chains per thread, 2 flop per FMA.  Thread 0 of every
+// block also reads the SM cycle counter and the nanosecond global timer around the loop, so the clock
+// the probe actually ran at is known (out[1 + 2 b], out[2 + 2 b] of block b).
+__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a, double b)
+{
+    double x[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) x[k] = (double)(threadIdx.x + k) * 1e-3;
+    long long c0 = 0, c1 = 0;
+    unsigned long long n0 = 0, n1 = 0;
+    if (threadIdx.x == 0) { c0 = clock64(); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(n0)); }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) x[k] = fma(x[k], a, b);
+    }
+    if (threadIdx.x == 0) { c1 = clock64(); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(n1)); }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s += x[k];
+    if (s == 123.456) out[0] = s;       // never true: keeps the loop alive
+    if (threadIdx.x == 0) { out[1 + 2 * blockIdx.x] = (double)(c1 - c0); out[2 + 2 * blockIdx.x] = (double)(n1 - n0); }
+}
+
+// max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x), and of the
+// tabulated a(P*), b(P*) against the direct formulas on (0, 3]
+__global__ void k_fastmath_test(int n, unsigned long long* err_bits, const double* __restrict__ tab)
+{
+    double er = 0.0, es = 0.0, eab = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        unsigned long long z = (unsigned long long)i * 0x9E3779B97F4A7C15ull + 0x2401152330ull;
+        z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
+        const double m = 1.0 + (double)(z >> 11) * (1.0 / 9007199254740992.0);       // [1, 2)
+        const double x = m * exp2((double)((int)(z & 255) - 128) * 0.78);            // ~1e-30 .. 1e30
+        const double r0 = 1.0 / x, s0 = sqrt(x);
+        er = fmax(er, fabs(mm::rcp(x) - r0) / r0);
+        es = fmax(es, fabs(mm::fsqrt(x) - s0) / s0);
+        const double P = 3.0 * (m - 1.0) + 1e-7 * (double)(z & 1023);   // (0, 3]: realizable p_dd
+        if (P > 0.0) {
+            double a0, b0, a1, b1;
+            ab_direct(P, &a0, &b0);
+            ab_eval(tab, P, a1, b1);
+            eab = fmax(eab, fmax(fabs(a1 - a0) / a0, fabs(b1 - b0) / b0));
+        }
+    }
+    const double ulp = 1.1102230246251565e-16;
+    atomic_max_pos(err_bits, er / ulp);
+    atomic_max_pos(err_bits + 1, es / ulp);
+    atomic_max_pos(err_bits + 2, eab / ulp);
+}
+
+
+double bits2d(unsigned long long b) { double d; memcpy(&d, &b, 8); return d; }
+
+}  // namespace
+
+extern "C" {
+
+int mm_measure_fp64_peak(void* stream, int repeats, double* tflops, double* sm_mhz)
+{
+    if (!tflops || repeats < 1) return -1;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
+    const int iters = 20000, blocks = sms * 8, threads = 256;
+    const size_t nout = 1 + 2 * (size_t)blocks;
+    double* d_out = nullptr;
+    if (cudaMalloc(&d_out, nout * sizeof(double)) != cudaSuccess) return -3;      // measurement scratch only
+    double* h_out = new double[nout];
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0, mhz = 0.0;
+    int rc = 0;
+    for (int r = 0; r < repeats + 1 && rc == 0; ++r) {            // first launch is the warm-up
+        cudaEventRecord(e0, st);
+        k_dfma_peak<<<blocks, threads, 0, st>>>(d_out, iters, 0.999999, 1e-6);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { rc = -3; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 16.0 * (double)iters * blocks * threads / (ms * 1e-3) * 1e-12;
+        if (r > 0 && tf > best) {
+            best = tf;
+            if (cudaMemcpy(h_out, d_out, nout * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = -3; break; }
+            double cyc = 0.0, ns = 0.0;
+            for (int b = 0; b < blocks; ++b) { cyc += h_out[1 + 2 * b]; ns += h_out[2 + 2 * b]; }
+            mhz = ns > 0.0 ? cyc / ns * 1e3 : 0.0;
+        }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out); delete[] h_out;
+    *tflops = best;
+    if (sm_mhz) *sm_mhz = mhz;
+    return rc;
+}
+
+int mm_selftest_fastmath(void* stream, int n, double* max_ulp)
+{
+    if (n < 1 || !max_ulp) return -1;
+    double* tab = nullptr;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* d = nullptr;
+    if (cudaMalloc(&d, 8 * sizeof(unsigned long long)) != cudaSuccess) return -3;   // measurement scratch only
+    if (cudaMalloc(&tab, AbTable::kDoubles * sizeof(double)) != cudaSuccess) { cudaFree(d); return -3; }
+    cudaMemsetAsync(d, 0, 8 * sizeof(unsigned long long), st);
+    k_ab_table<<<AbTable::kIntervals, 2, 0, st>>>(tab);
+    k_fastmath_test<<<296, 256, 0, st>>>(n, d, tab);
+    unsigned long long h[3] = {0, 0, 0};
+    cudaError_t e = cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d); cudaFree(tab);
+    if (e != cudaSuccess) return -3;
+    for (int k = 0; k < 3; ++k) max_ulp[k] = bits2d(h[k]);
+    return 0;
+}
+
+}  // extern "C"

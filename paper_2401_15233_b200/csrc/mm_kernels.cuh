@@ -30,6 +30,7 @@ struct Ctrl {
 // Boundary tables (device memory): conserved ghost states of the Dirichlet sides.
 struct BcSide {
     int type, nbands, has_default;
+    int maxwellian;                                   // W[k][0..4] = (rho, u_x, u_y, u_z, T): expanded by k_bc_table
     unsigned used;                                    // bit k: table entry k is selected by a ghost cell
     double lo[kMaxBands], hi[kMaxBands];
     double W[kMaxBands + 1][14];                      // primitive band states, [nbands] = default
@@ -103,9 +104,10 @@ __device__ __forceinline__ void cell_rate(const Params& p, const double (&U)[NM]
 template <int NM, bool PRIM>
 __global__ void k_pack(Params p, const double* __restrict__ src, double* __restrict__ dst)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.nx) return;
     const size_t plane = (size_t)p.rows * p.pitch, n = (size_t)p.nx * p.ny;
+    for (int j = blockIdx.y; j < p.ny; j += gridDim.y) {     // gridDim.y <= 65535 rows per sweep
     double a[NM], b[NM];
 #pragma unroll
     for (int m = 0; m < NM; ++m) a[m] = src[m * n + (size_t)j * p.nx + i];
@@ -117,14 +119,16 @@ __global__ void k_pack(Params p, const double* __restrict__ src, double* __restr
     }
 #pragma unroll
     for (int m = 0; m < NM; ++m) dst[m * plane + (size_t)(j + 2) * p.pitch + i + 2] = b[m];
+    }
 }
 
 template <int NM, bool PRIM>
 __global__ void k_unpack(Params p, const double* __restrict__ src, double* __restrict__ dst)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.nx) return;
     const size_t plane = (size_t)p.rows * p.pitch, n = (size_t)p.nx * p.ny;
+    for (int j = blockIdx.y; j < p.ny; j += gridDim.y) {
     double a[NM], b[NM];
 #pragma unroll
     for (int m = 0; m < NM; ++m) a[m] = src[m * plane + (size_t)(j + 2) * p.pitch + i + 2];
@@ -136,6 +140,7 @@ __global__ void k_unpack(Params p, const double* __restrict__ src, double* __res
     }
 #pragma unroll
     for (int m = 0; m < NM; ++m) dst[m * n + (size_t)j * p.nx + i] = b[m];
+    }
 }
 
 // Dirichlet tables: primitive -> conserved, and the constant ghost contribution to the CFL max
@@ -148,16 +153,31 @@ __global__ void k_bc_table(Params p, BcTable* tab, Ctrl* ctrl, int nsides)
     BcSide& b = tab->side[side];
     if (b.type != 2) return;
     const bool is_default = (k == b.nbands);
-    if (k > b.nbands || (is_default && !b.has_default) || !((b.used >> k) & 1u)) return;
+    if (k > b.nbands || (is_default && !b.has_default)) return;
     double W[NM], U[NM];
+    if (b.maxwellian) {
+        // Maxwellian of (rho, u, T): P = rho R_gas T (Eq 6), q = 0, R_iijj = 15 P^2/rho (L73),
+        // 5-moment r = 3 P^2/rho (L127)
+        const double rho = b.W[k][0], P = rho * p.R_gas * b.W[k][4];
 #pragma unroll
-    for (int m = 0; m < NM; ++m) W[m] = b.W[k][m];
+        for (int m = 0; m < NM; ++m) W[m] = 0.0;
+        W[0] = rho; W[1] = b.W[k][1];
+        if constexpr (NM == 5) { W[2] = P; W[4] = 3.0 * P * P / rho; }
+        else { W[2] = b.W[k][2]; W[3] = b.W[k][3]; W[4] = P; W[7] = P; W[9] = P; W[13] = 15.0 * P * P / rho; }
+#pragma unroll
+        for (int m = 0; m < NM; ++m) b.W[k][m] = W[m];
+    } else {
+#pragma unroll
+        for (int m = 0; m < NM; ++m) W[m] = b.W[k][m];
+    }
     if constexpr (NM == 5) prim2cons5(W, U); else prim2cons14<double>(W, U);
 #pragma unroll
     for (int m = 0; m < NM; ++m) b.U[k][m] = U[m];
+    // Every entry is converted (k_ghost may select any of them); only entries that some ghost cell
+    // actually takes (b.used, set at mm_create) count for the CFL maximum and the validity flags.
+    if (!((b.used >> k) & 1u)) return;
     double rate, speed; int bad = 0;
     cell_rate<NM>(p, U, rate, speed, bad);
-    // only entries that some ghost cell actually takes (b.used, set at mm_create) count
     atomic_max_pos(reinterpret_cast<unsigned long long*>(&ctrl->ghost_rate), rate);
     atomic_max_pos(reinterpret_cast<unsigned long long*>(&ctrl->ghost_speed), speed);
     if (bad) ctrl->bc_bad = 1;
@@ -379,23 +399,6 @@ k_step5(Params p, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl, int 
     if (do_rate) block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
 }
 
-// Register-resident DFMA loop: 16 independent chains per thread, 2 flop per FMA.
-__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a, double b)
-{
-    double x[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) x[k] = (double)(threadIdx.x + k) * 1e-3;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int k = 0; k < 16; ++k) x[k] = fma(x[k], a, b);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) s += x[k];
-    if (s == 123.456) out[0] = s;       // never true: keeps the loop alive
-}
-
-
 // cos(pi n / d) for integers n >= 0, d > 0, reduced exactly to the first quadrant so that the
 // argument handed to cospi is at most 1/2 and carries one rounding only
 __device__ inline double cos_quarter(int n, int d)
@@ -446,33 +449,6 @@ __global__ void k_ab_table(double* __restrict__ tab)
     }
     double* out = tab + i * AbTable::kStride;
     for (int j = 0; j < N; ++j) out[2 * j + f] = m[N - 1 - j];
-}
-
-// max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x), and of the
-// tabulated a(P*), b(P*) against the direct formulas on (0, 3]
-__global__ void k_fastmath_test(int n, unsigned long long* err_bits, const double* __restrict__ tab)
-{
-    double er = 0.0, es = 0.0, eab = 0.0;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        unsigned long long z = (unsigned long long)i * 0x9E3779B97F4A7C15ull + 0x2401152330ull;
-        z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
-        const double m = 1.0 + (double)(z >> 11) * (1.0 / 9007199254740992.0);       // [1, 2)
-        const double x = m * exp2((double)((int)(z & 255) - 128) * 0.78);            // ~1e-30 .. 1e30
-        const double r0 = 1.0 / x, s0 = sqrt(x);
-        er = fmax(er, fabs(rcp(x) - r0) / r0);
-        es = fmax(es, fabs(fsqrt(x) - s0) / s0);
-        const double P = 3.0 * (m - 1.0) + 1e-7 * (double)(z & 1023);   // (0, 3]: realizable p_dd
-        if (P > 0.0) {
-            double a0, b0, a1, b1;
-            ab_direct(P, &a0, &b0);
-            ab_eval(tab, P, a1, b1);
-            eab = fmax(eab, fmax(fabs(a1 - a0) / a0, fabs(b1 - b0) / b0));
-        }
-    }
-    const double ulp = 1.1102230246251565e-16;
-    atomic_max_pos(err_bits, er / ulp);
-    atomic_max_pos(err_bits + 1, es / ulp);
-    atomic_max_pos(err_bits + 2, eab / ulp);
 }
 
 }  // namespace mm

@@ -133,6 +133,7 @@ struct Params {               // per-solver constants, passed by value to the ke
     double dx, dy, x0, y0;
     double inv_tau_coef;      // MM_TAU_KN: 1/tau = inv_tau_coef * rho * sqrt(8 P /(pi rho))
     double inv_tau_const;     // MM_TAU_CONST: 1/tau
+    double R_gas;             // T = P/(rho R_gas): Maxwellian Dirichlet states (k_bc_table)
     int tau_model, limiter, shared_limiter, flux;
     int source_scheme;        // 0 explicit, 1 point-implicit (L348)
     int nx, ny, pitch, rows;  // padded array: rows x pitch doubles per moment, interior at (+2,+2)
@@ -145,8 +146,11 @@ struct Params {               // per-solver constants, passed by value to the ke
 
 __device__ __forceinline__ double clamp_sigma(double s, double lim)
 {
-    // sigma_bar = min(max(sigma, sigma_lim), 1)  (L163, L512; upper clamp: DESIGN.md R5)
-    return dmin(dmax(s, lim), 1.0);
+    // sigma_bar = min(max(sigma, sigma_lim), 1)  (L163, L512; upper clamp: DESIGN.md R5).  Written so that
+    // a NaN sigma (indefinite pressure tensor: negative radicand in Eq 21) stays NaN -- both comparisons
+    // are false -- and reaches the CFL reduction's failure flag.
+    const double t = s < lim ? lim : s;
+    return t > 1.0 ? 1.0 : t;
 }
 
 // ------------------------------------------------------------------ limiter (L262-266)

@@ -16,6 +16,7 @@ from . import build_ext
 SYS5_1D, SYS14_2D = 5, 14
 TAU_NONE, TAU_CONST, TAU_KN = 0, 1, 2
 BC_TRANSMISSIVE, BC_PERIODIC, BC_DIRICHLET = 0, 1, 2
+STATE_PRIMITIVE, STATE_MAXWELLIAN = 0, 1     # mm_bc.band_state: W[nmom] | (rho, u_x, u_y, u_z, T)
 LIM_NONE, LIM_MINMOD, LIM_VANALBADA = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
 SRC_EXPLICIT, SRC_POINT_IMPLICIT = 0, 1      # BGK source: forward Euler | point-implicit
@@ -26,11 +27,12 @@ MAX_BANDS = 8
 EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim", "mm_step",
            "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
            "mm_cfl_dt", "mm_get_dt_history", "mm_set_clock", "mm_decomposition", "mm_launch_count", "mm_profile_begin", "mm_profile_end",
-           "mm_measure_fp64_peak", "mm_selftest_fastmath", "mm_set_fast_path", "mm_fast_path_active",
+           "mm_set_fast_path", "mm_fast_path_active",
            "mm_destroy", "mm_strerror",
            "mm_batch5_workspace_bytes", "mm_batch5_create", "mm_batch5_set_state_prim", "mm_batch5_step",
            "mm_batch5_step_fixed_dt", "mm_batch5_advance_to", "mm_batch5_get_state", "mm_batch5_get_info",
            "mm_batch5_launch_count", "mm_batch5_destroy"]
+BENCH_EXPORTS = ["mm_measure_fp64_peak", "mm_selftest_fastmath"]          # include/mm_bench.h, libmm_bench.so
 
 _dp = C.POINTER(C.c_double)
 
@@ -40,6 +42,10 @@ class mm_grid(C.Structure):
                 ("x0", C.c_double), ("x1", C.c_double), ("y0", C.c_double), ("y1", C.c_double)]
 
 
+class mm_gas(C.Structure):
+    _fields_ = [("R_gas", C.c_double)]
+
+
 class mm_collision(C.Structure):
     _fields_ = [("model", C.c_int), ("tau", C.c_double), ("Kn", C.c_double),
                 ("L_ref", C.c_double), ("rho_ref", C.c_double)]
@@ -47,7 +53,7 @@ class mm_collision(C.Structure):
 
 class mm_bc(C.Structure):
     _fields_ = [("type", C.c_int), ("nbands", C.c_int), ("band_lo", _dp), ("band_hi", _dp),
-                ("band_W", _dp), ("default_W", _dp)]
+                ("band_W", _dp), ("default_W", _dp), ("band_state", C.c_int)]
 
 
 class mm_options(C.Structure):
@@ -75,7 +81,7 @@ def lib() -> C.CDLL:
     vp, i, d = C.c_void_p, C.c_int, C.c_double
     L.mm_workspace_bytes.restype, L.mm_workspace_bytes.argtypes = C.c_size_t, [C.POINTER(mm_grid)]
     L.mm_create.restype = i
-    L.mm_create.argtypes = [C.POINTER(vp), C.POINTER(mm_grid), C.POINTER(mm_collision),
+    L.mm_create.argtypes = [C.POINTER(vp), C.POINTER(mm_grid), C.POINTER(mm_gas), C.POINTER(mm_collision),
                             C.POINTER(mm_bc), C.POINTER(mm_options), vp, C.c_size_t]
     for name in ("mm_set_state", "mm_set_state_prim", "mm_get_state", "mm_get_state_prim"):
         f = getattr(L, name)
@@ -94,8 +100,6 @@ def lib() -> C.CDLL:
     L.mm_profile_begin.restype, L.mm_profile_begin.argtypes = i, [vp]
     L.mm_profile_end.restype = i
     L.mm_profile_end.argtypes = [vp, _dp, C.POINTER(C.c_longlong)]
-    L.mm_measure_fp64_peak.restype, L.mm_measure_fp64_peak.argtypes = i, [vp, i, _dp]
-    L.mm_selftest_fastmath.restype, L.mm_selftest_fastmath.argtypes = i, [vp, i, _dp]
     L.mm_set_fast_path.restype, L.mm_set_fast_path.argtypes = i, [vp, i]
     L.mm_fast_path_active.restype, L.mm_fast_path_active.argtypes = i, [vp]
     L.mm_destroy.restype, L.mm_destroy.argtypes = None, [vp]
@@ -116,6 +120,21 @@ def lib() -> C.CDLL:
     return L
 
 
+_bench_lib = None
+
+
+def bench_lib() -> C.CDLL:
+    """Load libmm_bench.so (include/mm_bench.h): the measurement hooks, kept out of the product library."""
+    global _bench_lib
+    if _bench_lib is None:
+        B = C.CDLL(str(build_ext.build_bench()))
+        vp, i = C.c_void_p, C.c_int
+        B.mm_measure_fp64_peak.restype, B.mm_measure_fp64_peak.argtypes = i, [vp, i, _dp, _dp]
+        B.mm_selftest_fastmath.restype, B.mm_selftest_fastmath.argtypes = i, [vp, i, _dp]
+        _bench_lib = B
+    return _bench_lib
+
+
 def _check(rc: int):
     if rc != OK:
         raise MMError(rc, lib().mm_strerror(rc).decode())
@@ -133,13 +152,14 @@ def mm_workspace_bytes(system: int, nx: int, ny: int = 1, extent=(0.0, 1.0, 0.0,
     return lib().mm_workspace_bytes(C.byref(g))
 
 
-def mm_measure_fp64_peak(repeats: int = 5, stream=None) -> float:
-    """Measured FP64 FMA peak of the current device in TFLOP/s (2 flop per FMA)."""
+def mm_measure_fp64_peak(repeats: int = 5, stream=None, with_clock: bool = False):
+    """Measured FP64 FMA peak of the current device in TFLOP/s (2 flop per FMA); with_clock: also the SM
+    clock (MHz) the probe ran at, from the kernel's own cycle counter and global timer."""
     import torch
     st = stream if stream is not None else torch.cuda.current_stream()
-    tf = C.c_double()
-    _check(lib().mm_measure_fp64_peak(C.c_void_p(st.cuda_stream), repeats, C.byref(tf)))
-    return tf.value
+    tf, mhz = C.c_double(), C.c_double()
+    _check(bench_lib().mm_measure_fp64_peak(C.c_void_p(st.cuda_stream), repeats, C.byref(tf), C.byref(mhz)))
+    return (tf.value, mhz.value) if with_clock else tf.value
 
 
 def mm_decomposition(nx: int, ny: int, zsym: bool = True, sms: int = 148):
@@ -155,14 +175,16 @@ def mm_selftest_fastmath(n: int = 1 << 22, stream=None):
     import torch
     st = stream if stream is not None else torch.cuda.current_stream()
     out = (C.c_double * 3)()
-    _check(lib().mm_selftest_fastmath(C.c_void_p(st.cuda_stream), n, out))
+    _check(bench_lib().mm_selftest_fastmath(C.c_void_p(st.cuda_stream), n, out))
     return tuple(out)
 
 
 class Solver:
     """mm_create ... mm_destroy around a torch-owned workspace.
 
-    `bcs`: 4 dicts (xlo, xhi, ylo, yhi): {"type": BC_*, "bands": [(lo, hi, W), ...], "default": W|None}.
+    `bcs`: 4 dicts (xlo, xhi, ylo, yhi): {"type": BC_*, "bands": [(lo, hi, W), ...], "default": W|None,
+    "state": STATE_PRIMITIVE (W = nmom primitives) | STATE_MAXWELLIAN (W = (rho, u_x, u_y, u_z, T))}.
+    `R_gas`: mm_gas.R_gas (T = P/(rho R_gas); only Maxwellian boundary states use it).
     State arrays are [nmom][ny][nx]; numpy arrays / CPU tensors go through the host path
     (on_device = 0), CUDA tensors through the device path (on_device = 1)."""
 
@@ -170,7 +192,7 @@ class Solver:
                  collision: Optional[dict] = None, bcs: Optional[Sequence[dict]] = None,
                  sigma_lim: float = 1e-4, ws_scale: float = 1.0, limiter: int = LIM_MINMOD,
                  shared_limiter: int = 0, flux: int = FLUX_HLL, source_scheme: int = SRC_EXPLICIT,
-                 time_scheme: int = TIME_EULER, device: str = "cuda:0", stream=None):
+                 time_scheme: int = TIME_EULER, R_gas: float = 1.0, device: str = "cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise MMError(ECUDA, "no CUDA device: the moment-method library has no CPU path")
@@ -193,10 +215,14 @@ class Solver:
             lo, hi = _darr([x[0] for x in bands]), _darr([x[1] for x in bands])
             bw = _darr([x[2] for x in bands]).reshape(-1)
             dflt = b.get("default")
-            dw = _darr(dflt, system) if dflt is not None else None
+            kind = b.get("state", STATE_PRIMITIVE)
+            nw = 5 if kind == STATE_MAXWELLIAN else system
+            if bw.size != nw * len(bands):
+                raise ValueError(f"boundary side {k}: band states must have {nw} entries each")
+            dw = _darr(dflt, nw) if dflt is not None else None
             keep += [lo, hi, bw, dw]
             arr[k] = mm_bc(b["type"], len(bands), lo.ctypes.data_as(_dp), hi.ctypes.data_as(_dp),
-                           bw.ctypes.data_as(_dp), dw.ctypes.data_as(_dp) if dw is not None else None)
+                           bw.ctypes.data_as(_dp), dw.ctypes.data_as(_dp) if dw is not None else None, kind)
         with torch.cuda.device(self.device):
             self._stream = stream if stream is not None else torch.cuda.current_stream()
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
@@ -205,7 +231,8 @@ class Solver:
             o = mm_options(sigma_lim, ws_scale, limiter, shared_limiter, flux, source_scheme, time_scheme,
                            C.c_void_p(self._stream.cuda_stream))
             h = C.c_void_p()
-            _check(L.mm_create(C.byref(h), C.byref(g), C.byref(c), arr, C.byref(o),
+            gas = mm_gas(R_gas)
+            _check(L.mm_create(C.byref(h), C.byref(g), C.byref(gas), C.byref(c), arr, C.byref(o),
                                C.c_void_p(self._ws_ptr), nbytes))
         self._h = h
         self.workspace_bytes = nbytes
@@ -372,6 +399,7 @@ class Batch5:
         if a.size != (self.ntubes if per_tube else 1) * 5 * self.nx:
             raise ValueError("bad state shape")
         _check(self._L.mm_batch5_set_state_prim(self._h, a.ctypes.data_as(C.c_void_p), int(per_tube), 0))
+        self._stream.synchronize()      # the host buffer may go away after this call (as Solver.set_state*)
 
     def step(self, n, cfl):
         _check(self._L.mm_batch5_step(self._h, n, cfl))

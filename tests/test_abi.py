@@ -17,8 +17,8 @@ def mm():
     return _mm
 
 
-def declared_functions():
-    text = (ROOT / "include" / "mm.h").read_text()
+def declared_functions(header="mm.h"):
+    text = (ROOT / "include" / header).read_text()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(mm_[a-z0-9_]+)\s*\(", text)))
 
@@ -29,6 +29,21 @@ def test_library_exports_every_declared_symbol(mm):
     lib = mm.lib()
     for n in names:
         assert getattr(lib, n) is not None
+    # the measurement hooks live in their own header and library (they allocate device scratch)
+    bnames = declared_functions("mm_bench.h")
+    assert set(bnames) == set(mm.BENCH_EXPORTS) and not set(bnames) & set(names)
+    blib = mm.bench_lib()
+    for n in bnames:
+        assert getattr(blib, n) is not None
+        assert not hasattr(lib, n)
+
+
+def test_product_library_never_allocates_device_memory():
+    """include/mm.h: "the library never allocates device memory" -- no cudaMalloc* in what builds libmm.so."""
+    from paper_2401_15233_b200 import build_ext
+    for f in build_ext.DEPS:
+        text = (build_ext.CSRC / f).resolve().read_text()
+        assert not re.search(r"\bcudaMalloc|\bcudaFree\b|cudaHostAlloc", text), f
 
 
 def test_binding_structs_match_header(mm):
@@ -37,7 +52,9 @@ def test_binding_structs_match_header(mm):
     assert "typedef struct { int system; int nx, ny; double x0, x1, y0, y1; } mm_grid;" in text
     assert [f[0] for f in mm.mm_grid._fields_] == ["system", "nx", "ny", "x0", "x1", "y0", "y1"]
     assert [f[0] for f in mm.mm_collision._fields_] == ["model", "tau", "Kn", "L_ref", "rho_ref"]
-    assert [f[0] for f in mm.mm_bc._fields_] == ["type", "nbands", "band_lo", "band_hi", "band_W", "default_W"]
+    assert [f[0] for f in mm.mm_bc._fields_] == ["type", "nbands", "band_lo", "band_hi", "band_W", "default_W", "band_state"]
+    assert "typedef struct { double R_gas; } mm_gas;" in text and [f[0] for f in mm.mm_gas._fields_] == ["R_gas"]
+    assert re.search(r"int mm_create\(mm_solver \*\*out, const mm_grid \*grid, const mm_gas \*gas, const mm_collision \*collision,", text)
     assert [f[0] for f in mm.mm_options._fields_] == ["sigma_lim", "ws_scale", "limiter", "shared_limiter", "flux", "source_scheme", "time_scheme", "stream"]
     for name, val in [("MM_SYS5_1D", 5), ("MM_SYS14_2D", 14), ("MM_MAX_BANDS", 8)]:
         assert re.search(rf"{name}\s*=?\s*{val}\b", text)
@@ -60,9 +77,13 @@ def test_workspace_bytes_and_argument_checks(mm):
     o = mm.mm_options(1e-4, 1.0, 1, 0, 0, 0, 0, None)
     b = (mm.mm_bc * 4)()
     h = C.c_void_p()
-    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(c), b, C.byref(o), None, 0) == mm.EWORKSPACE
+    gas = mm.mm_gas(287.0)
+    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(gas), C.byref(c), b, C.byref(o), None, 0) == mm.EWORKSPACE
+    assert lib.mm_create(C.byref(h), C.byref(g), None, C.byref(c), b, C.byref(o), None, 0) == mm.EWORKSPACE    # gas NULL: R = 1
+    gas.R_gas = 0.0
+    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(gas), C.byref(c), b, C.byref(o), None, 0) == mm.EINVAL
     o.sigma_lim = -1.0
-    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(c), b, C.byref(o), None, 0) == mm.EINVAL
+    assert lib.mm_create(C.byref(h), C.byref(g), None, C.byref(c), b, C.byref(o), None, 0) == mm.EINVAL
     assert lib.mm_step(None, 1, 0.4) == mm.EINVAL
     assert lib.mm_launch_count(None) == 0
 
@@ -82,7 +103,7 @@ def test_no_cpu_fallback(mm):
     b = (mm.mm_bc * 4)()
     h = C.c_void_p()
     n = lib.mm_workspace_bytes(C.byref(g))
-    assert lib.mm_create(C.byref(h), C.byref(g), C.byref(c), b, C.byref(o), C.c_void_p(4096), n) == mm.ECUDA
+    assert lib.mm_create(C.byref(h), C.byref(g), None, C.byref(c), b, C.byref(o), C.c_void_p(4096), n) == mm.ECUDA
     assert b"CUDA" in lib.mm_strerror(mm.ECUDA)
 
 

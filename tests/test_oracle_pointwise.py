@@ -559,3 +559,136 @@ def test_wavespeed_golden_spot_values(mmo):
             W = np.array([1.0, 0.0, 1.0, qd, 3 - 2 * sb + qd * qd / sb])      # sigma(q*, r*) = sb
             a, b = mmo.wavespeed5(W, 1e-12)
             assert b == pytest.approx(lmax, rel=1e-12) and a == pytest.approx(lmin, rel=1e-12)
+
+
+# --------------------------------------------- Eqs 25b-c: exact linear response at a Gaussian
+def _gaussian_linear_response(rho, Theta):
+    """At an anisotropic Gaussian (sigma = 0, q = 0) the 14-moment maximum-entropy family
+    f = exp(alpha . m(v)) (Eq 26) responds to a small heat flux dq, at fixed rho, u, P, through
+    d alpha in its odd generators (c_i, c_i c^2) only:  d<m_odd> = C d alpha, C = <m_odd m_odd^T>_G.
+    Hence dQ_ijk = <c_i c_j c_k m_odd> C^-1 (0, dq) and dS_i = <c_i c^4 m_odd> C^-1 (0, dq): Gaussian
+    moments up to degree 10, exact with an 8-node Gauss-Hermite rule.  Nothing of Eq 25 enters."""
+    Z, Wt = gh_nodes_3d(8)
+    c = Z @ np.linalg.cholesky(np.asarray(Theta, float)).T
+    m = rho * Wt
+    c2 = (c * c).sum(1)
+    modd = np.concatenate([c, c * c2[:, None]], 1)
+    Cinv = np.linalg.inv(np.einsum("n,na,nb->ab", m, modd, modd))
+    K = (np.einsum("n,ni,nj,nk,na->ijka", m, c, c, c, modd) @ Cinv)[..., 3:6]
+    Wm = (np.einsum("n,ni,na->ia", m, c * (c2 * c2)[:, None], modd) @ Cinv)[:, 3:6]
+    return K, Wm
+
+
+THETAS = [np.array([[1.2, 0.3, -0.1], [0.3, 0.7, 0.2], [-0.1, 0.2, 1.6]]),
+          np.diag([0.4, 1.0, 2.5]),
+          np.array([[0.9, -0.5, 0.0], [-0.5, 1.1, 0.0], [0.0, 0.0, 0.3]])]
+
+
+@pytest.mark.parametrize("Theta", THETAS)
+def test_eq25b_K_is_the_gaussian_linear_response(mmo, Theta):
+    """Eqs 22, 25b (L214, L228): K_ijkm is dQ_ijk/dq_m of the maximum-entropy distribution at the
+    Gaussian with the state's pressure tensor -- all 27 x 3 entries, to round-off, for ANY heat flux
+    and sigma (Eq 22 is linear in q and does not involve sigma).  Pins every coefficient and index
+    of Eq 25a-b on anisotropic, non-diagonal P."""
+    rho = 1.7
+    K, _ = _gaussian_linear_response(rho, Theta)
+    P = rho * Theta
+    q = np.array([0.3, -0.2, 0.5])
+    Rg = (2 * np.trace(P @ P) + np.trace(P) ** 2) / rho
+    for Rfac in (1.0, 1.3):
+        W = np.array([rho, 0.1, -0.2, 0.3, *[P[i, j] for i, j in SYM], *q, Rfac * Rg + 1.0])
+        _, _, Q, _, _ = mmo.closure14(W, SL)
+        np.testing.assert_allclose(Q, K @ q, rtol=0, atol=1e-12 * np.abs(Q).max())
+
+
+@pytest.mark.parametrize("Theta", THETAS)
+def test_eq25c_W_is_the_gaussian_linear_response(mmo, Theta):
+    """Eqs 24, 25c (L222, L230): at the Gaussian R (sigma = 0 -> sigma_bar = sigma_lim) and a heat flux
+    h << sigma_lim, Eq 24 reads S = W q + sqrt(sigma_lim) (2 P_jj/rho - W) q + O(h^3/sigma_lim^2),
+    and W_im must be dS_i/dq_m of the maximum-entropy family at that Gaussian.  The sqrt(sigma_lim)
+    term is removed by Richardson extrapolation over two limits; what is left agrees to 1e-7, so a
+    slip in any of the seven coefficients of Eq 25c (each moves W by percents) fails."""
+    rho = 1.7
+    _, Wm = _gaussian_linear_response(rho, Theta)
+    P = rho * Theta
+    Rg = (2 * np.trace(P @ P) + np.trace(P) ** 2) / rho
+    for q in (np.array([1e-14, 0, 0]), np.array([0, 1e-14, 0]), np.array([0, 0, 1e-14]), np.array([3e-15, -2e-15, 5e-15])):
+        W = np.array([rho, 0.1, -0.2, 0.3, *[P[i, j] for i, j in SYM], *q, Rg])
+        S = {}
+        for sl in (1e-8, 1e-10):
+            sg, sb, _, _, S[sl] = mmo.closure14(W, sl)
+            assert sg < 1e-12 and sb == sl
+        expect = Wm @ q
+        # plain: error ~ sqrt(sigma_lim)
+        assert np.abs(S[1e-10] - expect).max() <= 3e-5 * np.abs(expect).max()
+        # extrapolated in sqrt(sigma_lim): (1e-4 S(1e-10) ... ) -> W q
+        S0 = (1e-4 * S[1e-10] - 1e-5 * S[1e-8]) / (1e-4 - 1e-5)
+        assert np.abs(S0 - expect).max() <= 1e-7 * np.abs(expect).max()
+        # and the sqrt(sigma) coefficient itself is (2 P_jj / rho - W) q   (second term of Eq 24)
+        slope = (S[1e-8] - S[1e-10]) / (1e-4 - 1e-5)
+        np.testing.assert_allclose(slope, 2 * np.trace(P) / rho * q - expect, rtol=2e-5, atol=1e-6 * np.abs(expect).max())
+
+
+# ------------------------------------------------ upper clamp of sigma and radicand floor (R5, R6)
+def test_sigma_upper_clamp_uses_the_realizability_boundary(mmo):
+    """Reading R5: a state below the bound of Eq 19 (sigma > 1) is closed at sigma_bar = 1.  The closing
+    moments depend on the state only through (rho, P_ij, q_i, sigma_bar), so they must equal those of
+    the state with the same rho, P, q that sits ON the boundary (sigma = 1 exactly); the unclamped
+    sigma is still reported, and the wave speeds stay finite (sqrt(3 - 3 sigma) would be NaN)."""
+    for pdiag, h in (([1.0, 0.8, 1.2], [0.3, -0.2, 0.1]), ([0.6, 1.5, 0.9], [-0.8, 0.1, 0.4])):
+        W_in = state_from_sigma(pdiag, h, 1.0, rho=1.3, Ph=0.7, u=(0.2, -0.1, 0.3))
+        for sg_out in (1.2, 2.5):
+            W_out = state_from_sigma(pdiag, h, sg_out, rho=1.3, Ph=0.7, u=(0.2, -0.1, 0.3))
+            assert W_out[13] < W_in[13]                       # R below the bound of Eq 19
+            sg, sb, Q, R2, S = mmo.closure14(W_out, SL)
+            sg1, sb1, Q1, R21, S1 = mmo.closure14(W_in, SL)
+            assert sg == pytest.approx(sg_out, rel=1e-10) and sb == 1.0
+            assert sg1 == pytest.approx(1.0, rel=1e-10)
+            np.testing.assert_allclose(Q, Q1, rtol=1e-12, atol=1e-14)
+            np.testing.assert_allclose(R2, R21, rtol=1e-9, atol=1e-12)
+            np.testing.assert_allclose(S, S1, rtol=1e-9, atol=1e-12)
+            for d in range(3):
+                lmin, lmax = mmo.wavespeed14(W_out, d, SL)
+                lmin1, lmax1 = mmo.wavespeed14(W_in, d, SL)
+                assert math.isfinite(lmin) and math.isfinite(lmax) and lmin < W_out[1 + d] < lmax
+                assert lmin == pytest.approx(lmin1, rel=1e-9) and lmax == pytest.approx(lmax1, rel=1e-9)
+    # Eq 29 at sigma_bar = 1: E = C = 0, B = 1, Y = 1  =>  (a + b)/2 [zeta + sqrt(zeta^2 + 4 + qt^2/10)]
+    Pdd, qd, qt = 0.9, 0.4, 0.3
+    a = 1.4 * Pdd ** 1.1 * math.exp(-Pdd ** 2); b = 0.9 * Pdd * math.exp(-0.5 * Pdd ** 1.4)
+    zeta = qd + qt * (0.6 * Pdd ** 2 - 0.38 * Pdd + 0.35)
+    assert mmo.wavespeed14_star(Pdd, qd, qt, 1.0) == pytest.approx(0.5 * (a + b) * (zeta + math.sqrt(zeta ** 2 + 4 + qt ** 2 / 10)), rel=1e-13)
+    # 5-moment: r* < q*^2 + 1 (Eq 13 violated) -> sigma > 1 -> closed at 1: s* = q*^3 + 2 q* (two-point value)
+    W5 = np.array([1.0, 0.0, 1.0, 0.5, 0.9])
+    s5, sg5, sb5 = mmo.closure5(W5, SL)
+    assert sg5 > 1.0 and sb5 == 1.0 and s5 == pytest.approx(0.5 ** 3 + 2 * 0.5, rel=1e-13)
+    lmin, lmax = mmo.wavespeed5(W5, SL)
+    assert math.isfinite(lmin) and math.isfinite(lmax) and lmin < 0 < lmax
+
+
+def test_wavespeed14_radicand_floor(mmo):
+    """Reading R6: the radicand of Eq 29a, zeta^2 - 0.8 zeta sigma C + 4 sigma^2 Y + qt^2/10, is negative
+    at its minimum zeta = 0.4 sigma C with qt = 0 whenever 0.6 C < sqrt(B) < C, e.g. P* = 2.8, sigma = 0.1
+    (SURVEY.md section 8(c) point 6).  It is floored at 0: lambda* = (a sigma + b)/(2 sigma) zeta + E there --
+    finite, positive, and the limit of the neighbouring values where the radicand is positive."""
+    Pdd, sg = 2.8, 0.1
+    C = math.sqrt((3 - 3 * sg) * Pdd); E = 0.8 * C
+    B = 5 - 4 * math.sqrt(sg) + math.sqrt(10 - 16 * math.sqrt(sg) + 6 * sg)
+    assert 0.6 * C < math.sqrt(B) < C
+    Y = (math.sqrt(B) - E) ** 2
+    zeta = 0.4 * sg * C
+    assert zeta ** 2 - 0.8 * zeta * sg * C + 4 * sg ** 2 * Y < 0          # would be sqrt of a negative number
+    a = 1.4 * Pdd ** 1.1 * math.exp(-Pdd ** 2); b = 0.9 * Pdd * math.exp(-0.5 * Pdd ** 1.4)
+    lam = mmo.wavespeed14_star(Pdd, zeta, 0.0, sg)
+    assert math.isfinite(lam) and lam > 0
+    assert lam == pytest.approx((a * sg + b) / (2 * sg) * zeta + E, rel=1e-13)
+    # the two roots of the radicand bracket the floored interval; just outside it the value continues
+    disc = math.sqrt((0.4 * sg * C) ** 2 - 4 * sg ** 2 * Y)
+    z_hi = 0.4 * sg * C + disc
+    lam_out = mmo.wavespeed14_star(Pdd, z_hi * (1 + 1e-9), 0.0, sg)
+    lam_in = mmo.wavespeed14_star(Pdd, z_hi * (1 - 1e-9), 0.0, sg)
+    assert lam_out == pytest.approx(lam_in, rel=1e-3) and lam_out >= lam_in
+    # a full state through the laboratory-frame routine: finite and ordered
+    W = state_from_sigma([Pdd, (3 - Pdd) / 2, (3 - Pdd) / 2], [zeta, 0.0, 0.0], sg)
+    lmin, lmax = mmo.wavespeed14(W, 0, SL)
+    assert math.isfinite(lmin) and math.isfinite(lmax) and lmin < 0 < lmax
+    assert lmax == pytest.approx(lam, rel=1e-9)

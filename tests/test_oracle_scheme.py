@@ -425,3 +425,91 @@ def test_midpoint_is_second_order_in_time(mmo):
     U0 = oracle_solver(mmo, prob).get_state()
     for m in (0, 1, 2, 3):
         assert ref[m].sum() == pytest.approx(U0[m].sum(), rel=1e-12, abs=1e-12)
+
+
+# ------------------------------------------------- MUSCL face states, shared limiter (L262-266)
+# Hand-computed three-cell examples.  Every expected face value below is typed from the paper's
+# definition (L262: slope = psi (dm + dp)/2 with the symmetric limiter function; L266: "the same,
+# most stringent value of the limiter" for all primitive variables), not from the oracle.
+#   variable      Wm     W0     Wp      dm      dp     psi_minmod = 2 min/(|dm|+|dp|)   psi_vanAlbada = 2 dm dp/(dm^2+dp^2)
+#   a            1.0    2.0    4.0     1.0     2.0     2/3                               4/5
+#   b (flat)     0.0    0.0    0.0     0       0       imposes nothing (reading R14)
+#   c            2.0    2.5    2.625   0.5     0.125   2*0.125/0.625 = 2/5               0.125/0.265625 = 8/17
+#   d            0.4    0.5    0.6     0.1     0.1     1                                 1
+#   e            1.0    2.0    3.0     1.0     1.0     1                                 1
+FS_WM = [1.0, 0.0, 2.0, 0.4, 1.0]
+FS_W0 = [2.0, 0.0, 2.5, 0.5, 2.0]
+FS_WP = [4.0, 0.0, 2.625, 0.6, 3.0]
+FS_CENTRAL = [1.5, 0.0, 0.3125, 0.1, 1.0]          # (dm + dp)/2
+
+
+def test_face_states_shared_limiter_named_variable_sets_psi(mmo):
+    """Variable c is the most stringent one: psi = 2/5 (minmod) resp. 8/17 (van Albada) multiplies
+    the central slope of EVERY variable; the exactly flat variable b is skipped -- without the
+    skip rule its psi(0, 0) = 0 would flatten everything."""
+    for lim, psi in ((1, 2.0 / 5.0), (2, 8.0 / 17.0)):
+        lo, hi = mmo.face_states(lim, True, FS_WM, FS_W0, FS_WP)
+        for k in range(5):
+            half = 0.5 * psi * FS_CENTRAL[k]
+            assert lo[k] == pytest.approx(FS_W0[k] - half, rel=1e-15, abs=1e-16)
+            assert hi[k] == pytest.approx(FS_W0[k] + half, rel=1e-15, abs=1e-16)
+    # spelled out for minmod: psi = 0.4 -> half slopes 0.3, 0, 0.0625, 0.02, 0.2
+    lo, hi = mmo.face_states(1, True, FS_WM, FS_W0, FS_WP)
+    np.testing.assert_allclose(lo, [1.7, 0.0, 2.4375, 0.48, 1.8], rtol=1e-15, atol=0)
+    np.testing.assert_allclose(hi, [2.3, 0.0, 2.5625, 0.52, 2.2], rtol=1e-15, atol=0)
+
+
+def test_face_states_per_variable_limiter_differs(mmo):
+    """Per-variable mode on the same cells: each variable takes its own psi (minmod: the smaller
+    difference), so a = 2 -/+ 0.5, c = 2.5 -/+ 0.0625, d and e keep their full central slope."""
+    lo, hi = mmo.face_states(1, False, FS_WM, FS_W0, FS_WP)
+    np.testing.assert_allclose(lo, [1.5, 0.0, 2.4375, 0.45, 1.5], rtol=1e-15, atol=0)
+    np.testing.assert_allclose(hi, [2.5, 0.0, 2.5625, 0.55, 2.5], rtol=1e-15, atol=0)
+    lo, hi = mmo.face_states(2, False, FS_WM, FS_W0, FS_WP)           # van Albada: psi_k * central
+    np.testing.assert_allclose(hi - np.array(FS_W0), 0.5 * np.array([0.8, 0, 8 / 17, 1, 1]) * np.array(FS_CENTRAL),
+                               rtol=1e-14, atol=0)
+
+
+def test_face_states_shared_limiter_extremum_and_one_sided_flat(mmo):
+    """An extremum in ONE variable (dm dp < 0) gives psi = 0 for all of them (first order in that
+    cell); so does a variable that is flat on one side only (dm = 0, dp != 0: dm dp = 0 is not
+    > 0) -- only dm = dp = 0 exactly is exempt."""
+    for lim in (1, 2):
+        Wp = list(FS_WP); Wp[4] = 1.5                  # e: 1, 2, 1.5 -> local maximum
+        lo, hi = mmo.face_states(lim, True, FS_WM, FS_W0, Wp)
+        assert np.array_equal(lo, np.array(FS_W0)) and np.array_equal(hi, np.array(FS_W0))
+        Wm = list(FS_WM); Wm[3] = 0.5                  # d: 0.5, 0.5, 0.6 -> dm = 0, dp = 0.1
+        lo, hi = mmo.face_states(lim, True, Wm, FS_W0, FS_WP)
+        assert np.array_equal(lo, np.array(FS_W0)) and np.array_equal(hi, np.array(FS_W0))
+    # limiter off: zero slopes whatever the flag
+    lo, hi = mmo.face_states(0, True, FS_WM, FS_W0, FS_WP)
+    assert np.array_equal(lo, np.array(FS_W0)) and np.array_equal(hi, np.array(FS_W0))
+
+
+def test_face_states_shared_limiter_is_what_the_step_uses(mmo):
+    """The exported routine is the one inside the time step: one first-order-in-time step of a 1-D
+    5-moment problem with the shared limiter equals the update assembled here from face_states +
+    the pointwise flux / wave-speed / HLL functions (each pinned on its own)."""
+    rng = np.random.default_rng(11)
+    nx = 12
+    x = (np.arange(nx) + 0.5) / nx
+    W = np.stack([1 + 0.3 * np.sin(2 * np.pi * x), 0.2 * np.cos(2 * np.pi * x), 0.8 + 0.2 * np.sin(4 * np.pi * x),
+                  0.05 * np.sin(2 * np.pi * x + 1), 2.2 + 0.3 * np.cos(2 * np.pi * x)])
+    s = mmo.Solver(5, nx, 1, bcs=[dict(type=wl.BC_PERIODIC)] * 4, collision=dict(model=wl.TAU_NONE),
+                   limiter=wl.LIM_MINMOD, shared_limiter=1, flux=wl.FLUX_HLL)
+    s.set_state_prim(W[:, None, :])
+    U0 = s.get_state()[:, 0, :]
+    dt = 1e-3
+    s.step_fixed_dt(1, dt)
+    U1 = s.get_state()[:, 0, :]
+    lo = np.empty((5, nx)); hi = np.empty((5, nx))
+    for i in range(nx):
+        lo[:, i], hi[:, i] = mmo.face_states(wl.LIM_MINMOD, True, W[:, i - 1], W[:, i], W[:, (i + 1) % nx])
+    F = np.empty((5, nx))                               # F[:, i]: interface between cells i-1 and i
+    for i in range(nx):
+        WL, WR = hi[:, i - 1], lo[:, i]
+        a = mmo.wavespeed5(WL, 1e-4); b = mmo.wavespeed5(WR, 1e-4)
+        F[:, i] = mmo.numflux(wl.FLUX_HLL, mmo.flux5(WL, 1e-4), mmo.flux5(WR, 1e-4),
+                              mmo.prim2cons(WL), mmo.prim2cons(WR), a[0], a[1], b[0], b[1])
+    expect = U0 - dt * nx * (np.roll(F, -1, axis=1) - F)
+    np.testing.assert_allclose(U1, expect, rtol=1e-13, atol=1e-15)
