@@ -12,7 +12,7 @@ LIB = PKG / "libmm.so"                 # the product: include/mm.h
 BENCH_LIB = PKG / "libmm_bench.so"     # measurement / self-test hooks: include/mm_bench.h (allocates its own scratch)
 SOURCES = ["mm_api.cu"]
 BENCH_SOURCES = ["mm_bench.cu"]
-DEPS = ["mm_api.cu", "mm_kernels.cuh", "mm_strip14.cuh", "mm_batch5.cuh", "mm_physics.cuh", "../../include/mm.h"]
+DEPS = ["mm_api.cu", "mm_kernels.cuh", "mm_tm14.cuh", "mm_batch5.cuh", "mm_physics.cuh", "../../include/mm.h"]
 BENCH_DEPS = ["mm_bench.cu", "mm_kernels.cuh", "mm_physics.cuh", "../../include/mm_bench.h"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]

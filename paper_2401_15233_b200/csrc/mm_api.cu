@@ -2,7 +2,7 @@
 // kernel launches.  No arithmetic of the method runs here; there is no CPU fallback.
 #include "../../include/mm.h"
 #include "mm_kernels.cuh"
-#include "mm_strip14.cuh"
+#include "mm_tm14.cuh"
 #include "mm_batch5.cuh"
 
 #include <cstdio>
@@ -17,20 +17,11 @@ namespace {
 constexpr int kNT5 = 128;               // 5-moment cells per block
 constexpr int kRateNT = 256;
 
-// Resident blocks (= warps, one warp per block) per SM the two step-kernel variants are compiled
-// for: 8, which leaves each thread the full 255 registers (8 x 32 x 256 = the register file).
-// Measured on B200 (2048^2 z-symmetric step): 8 warps x 255 registers 1.30 ms; 10 x 200 1.36 ms;
-// 11 x 184 1.46 ms; 12 x 168 1.47 ms -- the closure has enough independent work per thread that
-// registers buy more than extra warps.  Shared memory allows 8 for both: strip buffers + the 9 KB
-// a/b table per block (z-symmetric), strip buffers alone (general, table through L1).
-constexpr size_t kSmemGen = ((size_t)kStripWPB * Mom<false>::warp_smem_doubles
-                             + (Mom<false>::table_in_smem ? AbTable::kDoubles : 0)) * sizeof(double);
-constexpr size_t kSmemZS = ((size_t)kStripWPB * Mom<true>::warp_smem_doubles + AbTable::kDoubles) * sizeof(double);
-constexpr int kBlocksByRegs = 8 / kStripWPB;
-constexpr int kBlocksGenSmem = (int)((227 * 1024) / (kSmemGen + 1024));
-constexpr int kBlocksZSSmem = (int)((227 * 1024) / (kSmemZS + 1024));
-constexpr int kMinBlocksGen = kBlocksGenSmem < kBlocksByRegs ? kBlocksGenSmem : kBlocksByRegs;
-constexpr int kMinBlocksZS = kBlocksZSSmem < kBlocksByRegs ? kBlocksZSSmem : kBlocksByRegs;
+// The 14-moment step kernel (mm_tm14.cuh) runs one block of Mom<ZS>::NW warps per SM; a warp is one
+// work item (strip x row chunk).
+constexpr size_t kSmemGen = Mom<false>::smem_bytes, kSmemZS = Mom<true>::smem_bytes;
+constexpr int kWarpsGen = Mom<false>::NW, kWarpsZS = Mom<true>::NW;
+static_assert(kSmemGen <= 227 * 1024 && kSmemZS <= 227 * 1024, "strip buffers exceed the shared memory of an SM");
 
 thread_local char g_cuda_msg[256] = "";
 
@@ -63,9 +54,9 @@ bool make_layout(const mm_grid* g, Layout* L)
     return true;
 }
 
-// Strips are kSW cells wide; rows are cut into nchunks chunks so that the nstrips * nchunks warp
-// items fill whole waves of the `slots` resident warps.  A chunk of n rows costs n + ~0.8 row
-// passes (one extra y-interface row and three extra row conversions).
+// Strips are kSW cells wide; rows are cut into nchunks chunks so that the nstrips * nchunks items (one
+// per warp) fill whole waves of the `slots` resident warps.  A chunk of n rows costs n + ~0.8 row
+// passes (one extra y-interface row and four extra row conversions).
 void choose_decomposition(int nx, int ny, int slots, int* nstrips, int* nchunks)
 {
     const int ns = (nx + kSW - 1) / kSW;
@@ -96,7 +87,7 @@ struct mm_solver {
     int has_state;
     long long hist_first;   // dt history is valid for steps >= hist_first (mm_set_clock moves it)
     long long launches;
-    int nstrips, nchunks[2];   // 14-moment work decomposition (mm_strip14.cuh): [general, z-symmetric]
+    int nstrips, nchunks[2];   // 14-moment work decomposition (mm_tm14.cuh): [general, z-symmetric]
     int time_scheme;        // MM_TIME_EULER | MM_TIME_MIDPOINT
     int zsym;               // state and boundary data have no z-odd moment: fast path applies
     int allow_fast;         // mm_set_fast_path
@@ -139,17 +130,15 @@ int launch_pass(mm_solver* s, int in, int out, const double* base, double dt_sca
     } else {
         const int fast = s->zsym && s->allow_fast;
         const int items = s->nstrips * s->nchunks[fast];
-        const int nb = (items + kStripWPB - 1) / kStripWPB;
         const bool ext = base != nullptr || dt_scale != 1.0 || !do_rate || s->p.source_scheme != 0;
-#define MM_LAUNCH_STRIP(ZSV, MINB, SMEM, NCH, EXTV)                                                   \
-    k_step14_strip<ZSV, MINB, EXTV><<<nb, 32 * kStripWPB, SMEM, s->stream>>>(                         \
-        s->p, s->U[in], s->U[out], s->ctrl, s->slot ^ 1, s->nstrips, NCH, base, dt_scale, do_rate)
-        if (fast) { if (ext) MM_LAUNCH_STRIP(true, kMinBlocksZS, kSmemZS, s->nchunks[1], true);
-                    else MM_LAUNCH_STRIP(true, kMinBlocksZS, kSmemZS, s->nchunks[1], false); }
-        else { if (ext) MM_LAUNCH_STRIP(false, kMinBlocksGen, kSmemGen, s->nchunks[0], true);
-               else MM_LAUNCH_STRIP(false, kMinBlocksGen, kSmemGen, s->nchunks[0], false); }
-#undef MM_LAUNCH_STRIP
-        MM_LAUNCHED(s, "k_step14_strip");
+#define MM_LAUNCH_TM(ZSV, EXTV)                                                                      \
+    k_step14_tm<ZSV, EXTV><<<(items + Mom<ZSV>::NW - 1) / Mom<ZSV>::NW, 32 * Mom<ZSV>::NW,             \
+                             Mom<ZSV>::smem_bytes, s->stream>>>(                                       \
+        s->p, s->U[in], s->U[out], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks[fast], base, dt_scale, do_rate)
+        if (fast) { if (ext) MM_LAUNCH_TM(true, true); else MM_LAUNCH_TM(true, false); }
+        else { if (ext) MM_LAUNCH_TM(false, true); else MM_LAUNCH_TM(false, false); }
+#undef MM_LAUNCH_TM
+        MM_LAUNCHED(s, "k_step14_tm");
     }
     return MM_OK;
 }
@@ -351,20 +340,20 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_gas* gas, const mm_
     if (nm == 14) {
         k_ab_table<<<AbTable::kIntervals, 2, 0, s->stream>>>((double*)(s->ws + L.off_tab));
         s->launches++;
-        e = cudaFuncSetAttribute(k_step14_strip<false, kMinBlocksGen, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
+        e = cudaFuncSetAttribute(k_step14_tm<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(k_step14_strip<false, kMinBlocksGen, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
+            e = cudaFuncSetAttribute(k_step14_tm<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(k_step14_strip<true, kMinBlocksZS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
+            e = cudaFuncSetAttribute(k_step14_tm<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(k_step14_strip<true, kMinBlocksZS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
-        if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaFuncSetAttribute(k_step14_strip)"); }
+            e = cudaFuncSetAttribute(k_step14_tm<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemZS);
+        if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaFuncSetAttribute(k_step14_tm)"); }
         int dev = 0, sms = 148;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         s->sms = sms;
-        choose_decomposition(grid->nx, grid->ny, sms * kMinBlocksGen * kStripWPB, &s->nstrips, &s->nchunks[0]);
-        choose_decomposition(grid->nx, grid->ny, sms * kMinBlocksZS * kStripWPB, &s->nstrips, &s->nchunks[1]);
+        choose_decomposition(grid->nx, grid->ny, sms * kWarpsGen, &s->nstrips, &s->nchunks[0]);
+        choose_decomposition(grid->nx, grid->ny, sms * kWarpsZS, &s->nstrips, &s->nchunks[1]);
         k_bc_table<14><<<4, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 4);
     } else {
         k_bc_table<5><<<2, kMaxBands + 1, 0, s->stream>>>(p, s->bc, s->ctrl, 2);
@@ -505,9 +494,9 @@ long long mm_launch_count(const mm_solver* s) { return s ? s->launches : 0; }
 int mm_decomposition(int nx, int ny, int zsym, int sms, int* nstrips, int* nchunks, int* warps_per_sm)
 {
     if (nx < 1 || ny < 1 || sms < 1 || !nstrips || !nchunks || !warps_per_sm) return MM_EINVAL;
-    const int w = (zsym ? kMinBlocksZS : kMinBlocksGen) * kStripWPB;
-    choose_decomposition(nx, ny, sms * w, nstrips, nchunks);
-    *warps_per_sm = w;
+    const int nw = zsym ? kWarpsZS : kWarpsGen;
+    choose_decomposition(nx, ny, sms * nw, nstrips, nchunks);
+    *warps_per_sm = nw;
     return MM_OK;
 }
 

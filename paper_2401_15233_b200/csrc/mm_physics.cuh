@@ -187,6 +187,32 @@ struct PsiShared {
     }
 };
 
+// a3: limited HALF slopes h_k of one cell along one direction from the primitives of its two neighbours
+// (L262-266): h = psi (dm + dp)/4 with one shared psi (L266), or h_k = limited_slope_k / 2 per variable.
+template <int NV>
+__device__ __forceinline__ void half_slopes(const Params& p, const double (&Wm)[NV], const double (&Wc)[NV],
+                                            const double (&Wp)[NV], double (&h)[NV])
+{
+    if (p.limiter == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) h[k] = 0.0;
+    } else if (p.shared_limiter) {
+        PsiShared pm;
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            const double dm = Wc[k] - Wm[k], dp = Wp[k] - Wc[k];
+            h[k] = dm + dp;
+            pm.add(p.limiter, dm, dp, h[k]);
+        }
+        const double q = 0.25 * pm.psi();
+#pragma unroll
+        for (int k = 0; k < NV; ++k) h[k] = q * h[k];
+    } else {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) h[k] = 0.5 * limited_slope(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
+    }
+}
+
 // ============================================================================ 5-moment
 // Eq 12 (L129-137).
 __device__ __forceinline__ void cons2prim5(const double (&U)[5], double (&W)[5])

