@@ -76,8 +76,9 @@ def opcount(write: bool = True) -> dict:
     if write:
         head = ("# FP64 operations per cell update of the CUDA path, counted at source level by\n"
                 "# `python -c 'from paper_2401_15233_b200 import build_ext; build_ext.opcount()'`\n"
-                "# (csrc/opcount_host.cpp; each + - * / sqrt and reciprocal = 1, FMA = 2, the a/b table evaluation\n"
-                "# 2 x 13 FMA + 2; no tile overhead).\n")
+                "# (csrc/opcount_host.cpp; each + - * / sqrt exp pow and reciprocal = 1, FMA = 2; no tile overhead).\n"
+                "# a(P*), b(P*) of Eq 29c-d are booked as the method's formulas (10 operations per call, SURVEY.md\n"
+                "# section 8(d)); the *_executed lines count the kernel's table evaluation (2 x 8 FMA + 2) instead.\n")
         OPCOUNT_TXT.write_text(head + out)
     return vals
 

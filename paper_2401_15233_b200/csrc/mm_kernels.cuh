@@ -20,6 +20,7 @@ struct Ctrl {
     double ghost_rate, ghost_speed;                   // constant part from Dirichlet ghost states
     long long bc_bad;                                 // a Dirichlet state has rho <= 0 or P <= 0
     long long bc_znz;                                 // a Dirichlet state has a non-zero z-odd moment
+    double sb_lim[4];                                 // sb_terms(sigma_lim): ss, isb, B, sqB (k_sb_lim, read back at create)
     long long steps;
     int bad[2];                                       // reduction saw rho<=0, P<=0 or non-finite
     int failed;                                       // sticky: stepping stopped (MM_ENONFINITE)
@@ -397,6 +398,13 @@ k_step5(Params p, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl, int 
         if (do_rate) cell_rate<NM>(p, Un, rate, speed, bad);
     }
     if (do_rate) block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
+}
+
+// sb_terms(sigma_lim) for Params::lim_* (one thread, at mm_create)
+__global__ void k_sb_lim(double sigma_lim, Ctrl* ctrl)
+{
+    const SbTerms t = sb_terms(sigma_lim);
+    ctrl->sb_lim[0] = t.ss; ctrl->sb_lim[1] = t.isb; ctrl->sb_lim[2] = t.B; ctrl->sb_lim[3] = t.sqB;
 }
 
 // cos(pi n / d) for integers n >= 0, d > 0, reduced exactly to the first quadrant so that the

@@ -80,10 +80,9 @@ __device__ __forceinline__ double rcp(double x)
 {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    const double e = fma(-x, r, 1.0);          // |e| <~ 2^-20
+    const double e = fma(-x, r, 1.0);          // |e| <~ 2^-20 (the seed sees the high word of x only)
     const double e2 = fma(e, e, e);            // e + e^2
-    const double e3 = fma(e2, e, e);           // e + e^2 + e^3
-    return fma(r, e3, r);                      // r (1 + e + e^2 + e^3): error e^4
+    return fma(r, e2, r);                      // r (1 + e + e^2): error e^3 ~ 2^-60
 }
 // sqrt(x) for x known to be positive and normal (P/rho, B >= 1): no zero / subnormal guard
 __device__ __forceinline__ double fsqrt_pos(double x)
@@ -141,6 +140,9 @@ struct Params {               // per-solver constants, passed by value to the ke
     // Literals whose low word is not zero (0.8, 0.1, ... of Eq 29, 1/3) cost two register moves per use
     // as immediates; as kernel parameters they are constant-bank operands of the FP64 instructions.
     double k08, k01, k06, k038, k035, k13;
+    // sb_terms(sigma_lim), evaluated once on the device at mm_create (k_sb_lim): a warp whose lanes all sit at
+    // sigma_bar = sigma_lim (every near-equilibrium region) takes these instead of three square roots per state
+    double lim_ss, lim_isb, lim_B, lim_sqB;
     __host__ void set_constants() { k08 = 0.8; k01 = 0.1; k06 = 0.6; k038 = 0.38; k035 = 0.35; k13 = 1.0 / 3.0; }
 };
 
@@ -477,32 +479,52 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
     t.sqB = fsqrt_pos(t.B);
     return t;
 }
+// sigma_bar = clamp(sigma) and its terms.  When every active lane of the warp is limited to sigma_lim the
+// terms are the constants sb_terms(sigma_lim) held in Params (bit-identical: same routine, same device).
+__device__ __forceinline__ SbTerms sb_terms_clamped(const Params& p, double sigma)
+{
+    const double sb = clamp_sigma(sigma, p.sigma_lim);
+#ifndef MM_OPCOUNT_HOST
+    if (__all_sync(__activemask(), sb == p.sigma_lim)) {
+        SbTerms t;
+        t.sb = sb; t.ss = p.lim_ss; t.isb = p.lim_isb; t.B = p.lim_B; t.sqB = p.lim_sqB;
+        return t;
+    }
+#endif
+    return sb_terms(sb);
+}
 
 // ---- a(P*) = 1.4 P*^1.1 exp(-P*^2) and b(P*) = 0.9 P* exp(-P*^1.4 / 2) of Eq 29c-d (L397-399)
-// They depend on the single variable P* = p_dd in (0, 3] and cost a pow and two exp per call,
+// They depend on the single variable P* = p_dd in (0, 3) and cost a pow and two exp per call,
 // six calls per cell update.  They are tabulated once per solver (k_ab_table, on the device, from
-// the formulas with libm pow / exp) as degree-13 Chebyshev interpolants re-expanded in powers of
-// the local coordinate t in [-1, 1], on 40 intervals read off the bits of P*:
-//   [2^-5, 2): 4 per octave, [2^e (1 + j/4), 2^e (1 + (j+1)/4));   [2, 4): 16 of width 1/8.
-// The branch point P* = 0 is at least 9 half-widths from every interval's centre (interpolation
-// error < 18^-14) and exp(-P*^2) varies by less than e^(+-1/2) over a half-width (its Chebyshev
-// coefficients fall below 1e-17 by degree 13); what remains is the round-off of 13 FMAs.
-// mm_selftest_fastmath measures it against the direct formulas.  Outside [2^-5, 4) and for NaN
-// the direct formulas are used.
+// the formulas with libm pow / exp) as degree-8 Chebyshev interpolants re-expanded in powers of
+// the local coordinate t in [-1, 1], on 224 intervals read off the bits of P*: 32 per octave on
+// [2^-5, 4),  [2^e (1 + j/32), 2^e (1 + (j+1)/32)),  i.e. the exponent and the top five mantissa bits
+// of P* are the interval index.  The branch point P* = 0 is at least 64 half-widths from every
+// interval's centre, and exp(-P*^2) varies by less than e^(+-1/4) over a half-width; the interpolation
+// error is below 2e-15 relative everywhere (what remains is the round-off of 8 FMAs).
+// mm_selftest_fastmath (include/mm_bench.h) measures it against the direct formulas.  Outside
+// [2^-5, 4) and for NaN the direct formulas are used.
 struct AbTable {
-    static constexpr int kLow = 24, kHigh = 16, kIntervals = kLow + kHigh, kDeg = 13;
+    static constexpr int kSubBits = 5, kSub = 1 << kSubBits;        // sub-intervals per octave
+    static constexpr int kOctLo = -5, kOctaves = 7;                 // [2^-5, 2^2)
+    static constexpr int kIntervals = kOctaves * kSub, kDeg = 8;
     static constexpr int kStride = 2 * (kDeg + 1);                  // (a_i, b_i) pairs, highest power first
     static constexpr int kDoubles = kIntervals * kStride;
-    static constexpr int kHiMin = (1023 - 5) << 20;                 // hi word of 2^-5, 2 and 4
-    static constexpr int kHiTwo = (1023 + 1) << 20, kHiMax = (1023 + 2) << 20;
+    static constexpr int kHiMin = (1023 + kOctLo) << 20;            // hi word of 2^-5 and of 4
+    static constexpr int kHiMax = (1023 + kOctLo + kOctaves) << 20;
+    static constexpr int kShift = 20 - kSubBits;                    // hi >> kShift = (exponent, top mantissa bits)
     // interval i: lower edge and 1 / half-width
     __host__ __device__ static double lower(int i)
     {
-        return i < kLow ? (1.0 + 0.25 * (i & 3)) * (1.0 / 32.0) * (double)(1 << (i >> 2)) : 2.0 + 0.125 * (i - kLow);
+        const int e = kOctLo + i / kSub, j = i % kSub;
+        const double two_e = e >= 0 ? (double)(1 << e) : 1.0 / (double)(1 << -e);
+        return two_e * (1.0 + (double)j / kSub);
     }
     __host__ __device__ static double inv_half(int i)
     {
-        return i < kLow ? 256.0 / (double)(1 << (i >> 2)) : 16.0;
+        const int e = kOctLo + i / kSub;                            // half-width 2^e / (2 kSub)
+        return e >= 0 ? (double)(2 * kSub) / (double)(1 << e) : (double)(2 * kSub) * (double)(1 << -e);
     }
 };
 #ifndef MM_OPCOUNT_HOST
@@ -515,11 +537,10 @@ __device__ __forceinline__ void ab_eval(const double* __restrict__ tab, double P
 {
     const int hi = __double2hiint(P);
     if (hi >= AbTable::kHiMin && hi < AbTable::kHiMax) {
-        const bool up = hi >= AbTable::kHiTwo;
-        const int idx = up ? AbTable::kLow + ((hi >> 16) & 15) : (hi >> 18) - (AbTable::kHiMin >> 18);
-        const double lo = __hiloint2double(hi & (up ? 0xFFFF0000 : 0xFFFC0000), 0);
-        // 1 / half-width: 16 on [2, 4), 2^(3 - e) on [2^e, 2^(e+1))
-        const double ih = __hiloint2double(up ? 0x40300000 : (2049 << 20) - (hi & 0x7FF00000), 0);
+        const int idx = (hi - AbTable::kHiMin) >> AbTable::kShift;
+        const double lo = __hiloint2double(hi & ~((1 << AbTable::kShift) - 1), 0);
+        // 1 / half-width = 2^(kSubBits + 1 - e): exponent field 1023 + kSubBits + 1 - (E - 1023)
+        const double ih = __hiloint2double(((2046 + AbTable::kSubBits + 1) << 20) - (hi & 0x7FF00000), 0);
         const double t = fma(P - lo, ih, -1.0);
         const double2* c = reinterpret_cast<const double2*>(tab + idx * AbTable::kStride);
         double2 q = c[0];
@@ -535,15 +556,17 @@ __device__ __forceinline__ void ab_eval(const double* __restrict__ tab, double P
     }
 }
 #else
+// Counted at the METHOD's operation count (pow and exp are one operation each):
+// a = 1.4 P^1.1 exp(-P^2) and b = 0.9 P exp(-P^1.4 / 2) are 5 + 5 operations, whatever the kernel's table
+// evaluation executes (2 x kDeg FMAs + 2) -- the roofline fraction cannot rise by adding instructions.
+// g_ab_executed_flops accumulates the executed count beside it.
+static long long g_ab_executed_flops = 0;
 __forceinline__ void ab_eval(const double* tab, double P, double& a, double& b)
-{   // same operations, counted: local coordinate + two degree-13 Horner evaluations
-    const double t = (P - 1.0) * 32.0 - 1.0;
-    double qa = tab[0], qb = tab[1];
-    for (int i = 1; i <= AbTable::kDeg; ++i) {
-        qa = qa * t + tab[2 * i];
-        qb = qb * t + tab[2 * i + 1];
-    }
-    a = qa; b = qb;
+{
+    (void)tab;
+    a = 1.4 * pow(P, 1.1) * exp(-(P * P));
+    b = 0.9 * P * exp(-0.5 * pow(P, 1.4));
+    g_ab_executed_flops += 2 * 2 * AbTable::kDeg + 2 - 10;      // what the table evaluation executes beyond the 10 counted
 }
 #endif
 
@@ -614,7 +637,7 @@ __device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[1
 {
     Star14<Z> s;
     nondim_sigma14<Z>(W, s);
-    const SbTerms t = sb_terms(clamp_sigma(s.sigma, p.sigma_lim));
+    const SbTerms t = sb_terms_clamped(p, s.sigma);
     const double sb = t.sb, isb = t.isb, ss = t.ss;
 
     const double I2 = 0.5 * (9.0 - s.t2), I3 = s.I3;
@@ -711,7 +734,7 @@ __device__ __forceinline__ bool cell_speeds14(const Params& p, const double (&W)
     if (!(W[0] > 0.0) || !(Ph > 0.0)) { sx = sy = 0.0; return false; }
     Star14<Z> s;
     nondim_sigma14<Z>(W, s);
-    const SbTerms t = sb_terms(clamp_sigma(s.sigma, p.sigma_lim));
+    const SbTerms t = sb_terms_clamped(p, s.sigma);
     double a, b;
     wavespeed14_x<Z>(p, s, t, W[1], a, b);
     sx = dmax(fabs(a), fabs(b));

@@ -89,24 +89,15 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// ---- tensor memory as lane-private scratch: N doubles of the calling lane at column `taddr` (each
+// ---- tensor memory as lane-private scratch: doubles of the calling lane at column `taddr` (each
 // thread of the warp touches its own lane; the instructions are warp-collective, .sync.aligned).
+// One double per instruction (32x32b.x2): its register pair is the operand as it stands, whereas the wider
+// shapes need their 8-32 registers contiguous and cost a register move per word (measured: 100 moves per
+// cell update with .x8 stores).
 __device__ __forceinline__ void tm_st2(unsigned taddr, double a)
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(__double2loint(a)),
                  "r"(__double2hiint(a)) : "memory");
-}
-__device__ __forceinline__ void tm_st4(unsigned taddr, double a, double b)
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr),
-                 "r"(__double2loint(a)), "r"(__double2hiint(a)), "r"(__double2loint(b)), "r"(__double2hiint(b)) : "memory");
-}
-__device__ __forceinline__ void tm_st8(unsigned taddr, const double* v)
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
-                 "r"(__double2loint(v[0])), "r"(__double2hiint(v[0])), "r"(__double2loint(v[1])), "r"(__double2hiint(v[1])),
-                 "r"(__double2loint(v[2])), "r"(__double2hiint(v[2])), "r"(__double2loint(v[3])), "r"(__double2hiint(v[3]))
-                 : "memory");
 }
 __device__ __forceinline__ double tm_ld2(unsigned taddr)
 {
@@ -114,44 +105,21 @@ __device__ __forceinline__ double tm_ld2(unsigned taddr)
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(taddr) : "memory");
     return __hiloint2double(hi, lo);
 }
-struct TmRaw4 { int r[8]; };
-__device__ __forceinline__ void tm_ld8(unsigned taddr, TmRaw4& q)
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                 : "=r"(q.r[0]), "=r"(q.r[1]), "=r"(q.r[2]), "=r"(q.r[3]), "=r"(q.r[4]), "=r"(q.r[5]), "=r"(q.r[6]), "=r"(q.r[7])
-                 : "r"(taddr) : "memory");
-}
 __device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
-// N doubles (N even or odd) to / from consecutive columns
 template <int N>
 __device__ __forceinline__ void tm_store(unsigned taddr, const double (&v)[N])
 {
-    int k = 0;
 #pragma unroll
-    for (; k + 4 <= N; k += 4) tm_st8(taddr + 2 * k, &v[k]);
-#pragma unroll
-    for (; k + 2 <= N; k += 2) tm_st4(taddr + 2 * k, v[k], v[k + 1]);
-    if (k < N) tm_st2(taddr + 2 * k, v[k]);
+    for (int k = 0; k < N; ++k) tm_st2(taddr + 2 * k, v[k]);
 }
 template <int N>
 __device__ __forceinline__ void tm_load(unsigned taddr, double (&v)[N])   // includes the wait
 {
-    constexpr int N4 = N / 4;
-    TmRaw4 q[N4 > 0 ? N4 : 1];
 #pragma unroll
-    for (int j = 0; j < N4; ++j) tm_ld8(taddr + 8 * j, q[j]);
-    double tail[3];
-#pragma unroll
-    for (int k = 4 * N4; k < N; ++k) tail[k - 4 * N4] = tm_ld2(taddr + 2 * k);
+    for (int k = 0; k < N; ++k) v[k] = tm_ld2(taddr + 2 * k);
     tm_wait_ld();
-#pragma unroll
-    for (int j = 0; j < N4; ++j)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) v[4 * j + i] = __hiloint2double(q[j].r[2 * i + 1], q[j].r[2 * i]);
-#pragma unroll
-    for (int k = 4 * N4; k < N; ++k) v[k] = tail[k - 4 * N4];
 }
 
 // Work decomposition: item = (strip, chunk); chunk c covers rows [c ny / nchunks, (c+1) ny / nchunks).
@@ -175,7 +143,9 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
     using M = Mom<ZS>;
     constexpr int NM = 14, NV = M::NV, NF = 2 * NV + 2, RS = NV * kRW;   // RS: doubles per staged row
     extern __shared__ __align__(16) double smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // the warp index through a shuffle: the compiler then knows it is warp-uniform and keeps what derives
+    // from it (buffer bases, tensor-memory addresses) in uniform registers
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
 
     // the block's copy of the a(P*), b(P*) table (Eq 29c-d), and its tensor-memory allocation
     Params p = pg;
@@ -192,7 +162,8 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
     const unsigned tm_base = *tm_slot;
     p.ab = smem;
     // this warp's 32 lanes x 128 columns: lane quarter warp % 4 (the only one the warp may touch)
-    const unsigned tm = tm_base + ((unsigned)(32 * (warp & 3)) << 16) + (unsigned)(M::tm_stride * (warp >> 2));
+    const unsigned tm = __shfl_sync(0xffffffffu, tm_base + ((unsigned)(32 * (warp & 3)) << 16)
+                                                     + (unsigned)(M::tm_stride * (warp >> 2)), 0);
 
     const int item = blockIdx.x * M::NW + warp;
     bool work = item < nstrips * nchunks;
