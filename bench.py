@@ -36,25 +36,31 @@ CFL = 0.4
 
 
 def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14):
-    """Algorithmic FP64 operations per cell update (each + - * / sqrt exp log = 1).
-    -> (count of the formulation the CUDA path runs, count of the oracle's naive restatement).
-    The roofline line uses the FIRST (smaller) number: flops the kernel does not execute are not
-    credited to it.  Both are produced by committed counting builds, not typed in."""
+    """Algorithmic FP64 operations per cell update (each + - * / sqrt exp
+    pow = 1, so a(P*), b(P*) of Eq 29c-d are 10 per call whatever the kernel's table evaluation executes).
+    -> (count of the formulation the CUDA path runs, the same with the table evaluation as executed,
+        count of the oracle's naive restatement).
+    The roofline line uses the FIRST (smallest) number: flops the kernel does not execute, or executes
+    only because of an implementation choice, are not credited to it.  All are produced by committed
+    counting builds, not typed in."""
     from paper_2401_15233_b200 import build_ext
-    k = build_ext.read_opcount()[f"kernel_flops_per_cell_update_{system}_" + ("zsym_" if zsym and system == 14 else "")
-                                 + ("shared_limiter" if shared_limiter else "per_variable_limiter")]
+    key = (f"kernel_flops_per_cell_update_{system}_" + ("zsym_" if zsym and system == 14 else "")
+           + ("shared_limiter" if shared_limiter else "per_variable_limiter"))
+    oc = build_ext.read_opcount()
+    k = oc[key]
     o = None
     for line in (ROOT / "tests" / "golden" / "oracle_opcount.txt").read_text().splitlines():
         if line.startswith(f"flops_per_cell_update_{system} "):
             o = float(line.split()[1])
-    return float(k), o
+    return float(k), float(oc.get(key + "_executed", k)), o
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None where no capture of that configuration exists).
 NCU_TRAFFIC_BYTES = {
-    ("k_step14_strip<zsym>", 2048): (351.97e6 + 423.15e6, "profiles/r1m_k_step14_strip_zsym.md"),
+    ("k_step14_tm<zsym>", 2048): (356.73e6 + 421.49e6, "profiles/r2_k_step14_tm_zsym.md"),
 }
+FP64_LANES_PER_SM = 64      # DFMA lanes of a B200 SM: nominal peak = SMs x 64 x 2 flop x SM clock
 
 
 def peaks() -> dict:
@@ -150,10 +156,16 @@ def workload(n: int, kn: float) -> dict:
     return WORKLOADS[WORKLOAD][0](n, kn)
 
 
-def time_oracle(n: int, kn: float, steps: int, warmup: int = 0, nthreads: int = 0):
+def time_oracle(n: int, kn: float, steps: int, warmup: int = 0, nthreads: int = 0, ny: int = 0):
     """Oracle (as it stands) on an n x n instance of the workload: cell-updates/s, threads."""
     from oracle import mmo
     prob = workload(n, kn)
+    if ny and ny < prob["ny"]:          # a band of rows around the lower jet (same cells, same boundary data)
+        j0 = max(0, min(prob["ny"] - ny, int(0.35 * prob["ny"]) - ny // 2))
+        y0, y1 = prob["extent"][2], prob["extent"][3]
+        h = (y1 - y0) / prob["ny"]
+        prob = dict(prob, ny=ny, W0=np.ascontiguousarray(prob["W0"][:, j0:j0 + ny]),
+                    extent=(prob["extent"][0], prob["extent"][1], y0 + j0 * h, y0 + (j0 + ny) * h))
     so = mmo.Solver(prob["system"], prob["nx"], prob["ny"], extent=prob["extent"],
                     collision=prob["collision"], bcs=prob["bcs"], nthreads=nthreads, **prob["options"])
     so.set_state_prim(prob["W0"])
@@ -266,6 +278,10 @@ def run_gpu(args):
         s.set_fast_path(False)
     # ---- device-resident timing: K steps, inputs in HBM (two 470 MB copies >> 126 MB L2)
     s.set_state_prim(W_dev)
+    developed = None
+    if args.developed_t > 0.0:          # timed window on a developed state: CFL steps to t first
+        s.advance_to(args.developed_t, CFL)
+        developed = s.info(check=False)
     s.step(W, CFL)
     barrier()
     l0 = s.launches
@@ -304,8 +320,11 @@ def run_gpu(args):
     finite = bool(torch.isfinite(U_host).all())
 
     if rank == 0:
-        fpc, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]), s.fast_path_active, nm)
-        peak_tf = mm.mm_measure_fp64_peak(5)
+        fpc, fpc_exec, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]), s.fast_path_active, nm)
+        # the probe also reports the SM clock it ran at (cycle counter / global timer inside the kernel)
+        peak_tf, peak_mhz = mm.mm_measure_fp64_peak(5, with_clock=True)
+        sms = torch.cuda.get_device_properties(local).multi_processor_count
+        nominal_tf = sms * FP64_LANES_PER_SM * 2.0 * (peak_mhz or 0.0) * 1e6 * 1e-12
         kern_avg_ms = kern_ms / max(kern_n, 1)
         achieved_tf = fpc * cells / (kern_avg_ms * 1e-3) * 1e-12
         pk = peaks()
@@ -313,11 +332,17 @@ def run_gpu(args):
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             v, threads, secs = time_oracle(args.ref_n, args.kn, args.cpu_steps)
+            # the paper's own baseline is ONE core: the same oracle, one thread, on a
+            # 128-row band of the same instance
+            v1, t1, s1 = time_oracle(args.ref_n, args.kn, args.cpu_steps_single, nthreads=1, ny=128)
             cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                    "sample": f"{args.ref_n}x{args.ref_n} instance of the same workload, "
-                             f"{args.cpu_steps} CFL steps ({secs:.1f} s)"}
+                             f"{args.cpu_steps} CFL steps ({secs:.1f} s)",
+                   "single_thread": {"value": v1, "unit": UNIT, "cores": t1,
+                                     "sample": f"{args.ref_n}x128 band of that instance around the lower jet, "
+                                               f"{args.cpu_steps_single} CFL steps ({s1:.1f} s)"}}
         kernel_name = ("k_step5" if nm == 5 else
-                       "k_step14_strip<zsym>" if s.fast_path_active else "k_step14_strip<general>")
+                       "k_step14_tm<zsym>" if s.fast_path_active else "k_step14_tm<general>")
         traffic, traffic_src = NCU_TRAFFIC_BYTES.get((kernel_name, n), (None, None)) if WORKLOAD == "baseline" else (None, None)
         out = {
             "metric": METRIC if nm == 14 else "cell-updates/s (fp64, 5-moment 1-D)",
@@ -328,7 +353,10 @@ def run_gpu(args):
                        "cells": cells, "l2": (f"inputs larger than L2 (2 x {nbytes_state / 1e6:.0f} MB state copies)" if nbytes_state > 126e6
                               else f"L2-resident state ({nbytes_state / 1e6:.2f} MB): not a bandwidth measurement"),
                        "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "t_end": info["t"], "state_finite": finite},
+                       "t_end": info["t"], "state_finite": finite,
+                       "window": (f"developed state: {developed['steps']} CFL steps to t = {developed['t']:.4g} before "
+                                  f"the warm-up (status {developed['status']})" if developed else
+                                  "starting state of the config + warm-up steps")},
             "clocks": clk.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes_state / K,
                     "d2h_bytes_per_step": nbytes_state / K,
@@ -341,8 +369,13 @@ def run_gpu(args):
                          "traffic_source": traffic_src, "algorithmic_bytes_per_launch": 16.0 * nm * cells,
                          "kernel": kernel_name,
                          "kernel_ms": kern_avg_ms,
-                         "flops_per_cell_update": fpc, "flops_per_cell_update_oracle": fpc_oracle,
-                         "peak_source": "FP64 DFMA loop measured in this run (mm_measure_fp64_peak)",
+                         "flops_per_cell_update": fpc, "flops_per_cell_update_executed": fpc_exec,
+                         "flops_per_cell_update_oracle": fpc_oracle,
+                         "flops_convention": "SURVEY.md 8(d): + - * / sqrt exp pow = 1 each, FMA = 2; a(P*), b(P*) of "
+                                             "Eq 29c-d booked as the method's formulas, not as the table evaluation",
+                         "peak_source": "FP64 DFMA loop measured in this run (mm_measure_fp64_peak, libmm_bench.so)",
+                         "peak_sm_mhz": peak_mhz, "peak_nominal": nominal_tf,
+                         "frac_of_nominal": achieved_tf / nominal_tf if nominal_tf else None,
                          "hbm_algorithmic_gbs": hbm_gbs, "hbm_peak_gbs": pk.get("hbm_gbs"),
                          "hbm_frac": hbm_gbs / pk["hbm_gbs"] if pk.get("hbm_gbs") else None},
             "cpu_baseline": cpu,
@@ -363,6 +396,10 @@ def main():
     ap.add_argument("--ref-n", type=int, default=512, help="grid of the bounded oracle sample")
     ap.add_argument("--cpu-steps", type=int, default=250,
                     help="oracle steps of the cpu_baseline leg (~15 s on 16 cores at 512^2)")
+    ap.add_argument("--cpu-steps-single", type=int, default=16,
+                    help="oracle steps of the single-thread leg (~10 s on a 512 x 128 band)")
+    ap.add_argument("--developed-t", type=float, default=0.0,
+                    help="advance to this time with CFL steps before the warm-up (developed-state window)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tubes", type=int, default=4096, help="--workload sod5-batch: number of tubes")
     ap.add_argument("--workload", default="baseline", choices=sorted(WORKLOADS) + ["sod5-batch"],

@@ -533,27 +533,35 @@ __device__ __noinline__ void ab_direct(double P, double* a, double* b)
     *a = 1.4 * pow(P, 1.1) * exp(-(P * P));
     *b = 0.9 * P * exp(-0.5 * pow(P, 1.4));
 }
-__device__ __forceinline__ void ab_eval(const double* __restrict__ tab, double P, double& a, double& b)
+__device__ __forceinline__ bool ab_in_table(double P)
 {
     const int hi = __double2hiint(P);
-    if (hi >= AbTable::kHiMin && hi < AbTable::kHiMax) {
-        const int idx = (hi - AbTable::kHiMin) >> AbTable::kShift;
-        const double lo = __hiloint2double(hi & ~((1 << AbTable::kShift) - 1), 0);
-        // 1 / half-width = 2^(kSubBits + 1 - e): exponent field 1023 + kSubBits + 1 - (E - 1023)
-        const double ih = __hiloint2double(((2046 + AbTable::kSubBits + 1) << 20) - (hi & 0x7FF00000), 0);
-        const double t = fma(P - lo, ih, -1.0);
-        const double2* c = reinterpret_cast<const double2*>(tab + idx * AbTable::kStride);
-        double2 q = c[0];
+    return hi >= AbTable::kHiMin && hi < AbTable::kHiMax;
+}
+// table value, no branch: for P outside [2^-5, 4) the interval index is clamped and the result is NOT a(P), b(P)
+// -- the caller tests ab_in_table and redoes those (rare) states with the direct formulas
+__device__ __forceinline__ void ab_table(const double* __restrict__ tab, double P, double& a, double& b)
+{
+    const int hi = __double2hiint(P);
+    const int idx = min(max((hi - AbTable::kHiMin) >> AbTable::kShift, 0), AbTable::kIntervals - 1);
+    const double lo = __hiloint2double(hi & ~((1 << AbTable::kShift) - 1), 0);
+    // 1 / half-width = 2^(kSubBits + 1 - e): exponent field 1023 + kSubBits + 1 - (E - 1023)
+    const double ih = __hiloint2double(((2046 + AbTable::kSubBits + 1) << 20) - (hi & 0x7FF00000), 0);
+    const double t = fma(P - lo, ih, -1.0);
+    const double2* c = reinterpret_cast<const double2*>(tab + idx * AbTable::kStride);
+    double2 q = c[0];
 #pragma unroll
-        for (int i = 1; i <= AbTable::kDeg; ++i) {
-            const double2 ci = c[i];
-            q.x = fma(q.x, t, ci.x);
-            q.y = fma(q.y, t, ci.y);
-        }
-        a = q.x; b = q.y;
-    } else {
-        ab_direct(P, &a, &b);
+    for (int i = 1; i <= AbTable::kDeg; ++i) {
+        const double2 ci = c[i];
+        q.x = fma(q.x, t, ci.x);
+        q.y = fma(q.y, t, ci.y);
     }
+    a = q.x; b = q.y;
+}
+__device__ __forceinline__ void ab_eval(const double* __restrict__ tab, double P, double& a, double& b)
+{
+    if (ab_in_table(P)) ab_table(tab, P, a, b);
+    else ab_direct(P, &a, &b);
 }
 #else
 // Counted at the METHOD's operation count (pow and exp are one operation each):
@@ -574,11 +582,15 @@ __forceinline__ void ab_eval(const double* tab, double P, double& a, double& b)
 // heat flux along (hd) and across (qt2 = sum of squares of the other two), sigma_bar terms.
 // a(P*), b(P*) come from the table (ab_eval); Y = B + E^2 - 2 E sqrt(B)
 // is evaluated as (sqrt(B) - E)^2; the radicand is floored at 0 (R6).
+template <bool TABLE_ONLY = false>
 __device__ __forceinline__ void ws14_dir(const Params& p, double Pdd, double hd,
                                          double qt, double qt2, const SbTerms& t, double& lam_max,
                                          double& lam_min_neg)
 {
     double a, b;
+#ifndef MM_OPCOUNT_HOST
+    if constexpr (TABLE_ONLY) ab_table(p.ab, Pdd, a, b); else
+#endif
     ab_eval(p.ab, Pdd, a, b);
     const double C = fsqrt_pos((3.0 - 3.0 * t.sb) * Pdd + kTiny);
     const double E = p.k08 * C;
@@ -594,14 +606,14 @@ __device__ __forceinline__ void ws14_dir(const Params& p, double Pdd, double hd,
 }
 
 // lambda_min / lambda_max along x of an (index-swapped for y) state, Eqs 28-31 (L388-411).
-template <class Z>
+template <class Z, bool TABLE_ONLY = false>
 __device__ __forceinline__ void wavespeed14_x(const Params& p, const Star14<Z>& s,
                                               const SbTerms& t, double ux, double& lmin, double& lmax)
 {
     double a, b, qt;                                                 // Eq 28: qtilde >= 0 (R7)
     const double qt2 = s.hy * s.hy + s.hz * s.hz;
     if constexpr (std::is_same<Z, zero_t>::value) qt = fabs(s.hy); else qt = fsqrt(qt2);
-    ws14_dir(p, s.pxx, s.hx, qt, qt2, t, a, b);
+    ws14_dir<TABLE_ONLY>(p, s.pxx, s.hx, qt, qt2, t, a, b);
     const double kc = p.ws_scale * s.c;
     lmax = ux + kc * a; lmin = ux - kc * b;
 }
@@ -630,14 +642,37 @@ __device__ __forceinline__ void wavespeed14_y(const Params& p, const Star14<Z>& 
 // I2 = (9 - t2)/2, I3 = det p), so M = m2 p^2 + m1 p + m0.
 // The flux polynomials are written as F = u_x U + (pressure / heat-flux / closure terms).
 // z-odd slots of F and U are left untouched when Z = zero_t.
+// The evaluation in two parts, so that the step kernel can run part B of one face next to part A of the
+// other in one basic block (the latency-bound reciprocal / square-root chains of A against the
+// multiply-add-rich B):
+//   A: dimensionless state, sigma, sigma_bar terms, wave speeds (Eqs 6, 21, 28-31);
+//   B: closing moments, flux, conserved state (Eqs 22-25, 16).
 template <class Z>
-__device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[14],
-                                            double (&F)[14], double (&U)[14], double& lmin,
-                                            double& lmax)
+struct FaceA { Star14<Z> s; SbTerms t; };
+
+// TABLE_ONLY: a(P*), b(P*) from the table without the range test (no branch inside the block); the caller
+// must check ab_in_table(a.s.pxx) afterwards and call face14_speeds_direct where it fails.
+template <class Z, bool TABLE_ONLY = false>
+__device__ __forceinline__ void eval_face14_A(const Params& p, const double (&W)[14], FaceA<Z>& a,
+                                              double& lmin, double& lmax)
 {
-    Star14<Z> s;
-    nondim_sigma14<Z>(W, s);
-    const SbTerms t = sb_terms_clamped(p, s.sigma);
+    nondim_sigma14<Z>(W, a.s);
+    a.t = sb_terms_clamped(p, a.s.sigma);
+    wavespeed14_x<Z, TABLE_ONLY>(p, a.s, a.t, W[1], lmin, lmax);
+}
+template <class Z>
+__device__ __forceinline__ void face14_speeds_direct(const Params& p, const double (&W)[14], const FaceA<Z>& a,
+                                                     double& lmin, double& lmax)
+{
+    wavespeed14_x<Z, false>(p, a.s, a.t, W[1], lmin, lmax);
+}
+
+template <class Z>
+__device__ __forceinline__ void eval_face14_B(const Params& p, const double (&W)[14], const FaceA<Z>& fa,
+                                              double (&F)[14], double (&U)[14])
+{
+    const Star14<Z>& s = fa.s;
+    const SbTerms& t = fa.t;
     const double sb = t.sb, isb = t.isb, ss = t.ss;
 
     const double I2 = 0.5 * (9.0 - s.t2), I3 = s.I3;
@@ -721,7 +756,16 @@ __device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[1
                      + uy * (uy * Qyyx + 2.0 * uz * Qyzx) + uz * uz * Qzzx;
     F[13] = ux * U[13] + 2.0 * u2 * k1 + 4.0 * (uuQ + ux * Rx + uy * Ry + uz * Rz) + Sx;   // 16e
 
-    wavespeed14_x<Z>(p, s, t, ux, lmin, lmax);
+}
+
+template <class Z>
+__device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[14],
+                                            double (&F)[14], double (&U)[14], double& lmin,
+                                            double& lmax)
+{
+    FaceA<Z> a;
+    eval_face14_A<Z>(p, W, a, lmin, lmax);
+    eval_face14_B<Z>(p, W, a, F, U);
 }
 
 // max(|lmin|,|lmax|) along x and y of a cell-centre state, for the CFL reduction (L434).

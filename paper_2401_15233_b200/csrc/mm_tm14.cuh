@@ -93,7 +93,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // thread of the warp touches its own lane; the instructions are warp-collective, .sync.aligned).
 // One double per instruction (32x32b.x2): its register pair is the operand as it stands, whereas the wider
 // shapes need their 8-32 registers contiguous and cost a register move per word (measured: 100 moves per
-// cell update with .x8 stores).
+// cell update with .x8 stores; same run time either way).
 __device__ __forceinline__ void tm_st2(unsigned taddr, double a)
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(__double2loint(a)),
