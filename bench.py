@@ -58,7 +58,7 @@ def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14):
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None where no capture of that configuration exists).
 NCU_TRAFFIC_BYTES = {
-    ("k_step14_tm<zsym>", 2048): (356.73e6 + 421.49e6, "profiles/r2_k_step14_tm_zsym.md"),
+    ("k_step14_tm<zsym>", 2048): (357.10e6 + 423.01e6, "profiles/r2a_k_step14_tm_zsym.md"),
 }
 FP64_LANES_PER_SM = 64      # DFMA lanes of a B200 SM: nominal peak = SMs x 64 x 2 flop x SM clock
 

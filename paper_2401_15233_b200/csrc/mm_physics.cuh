@@ -505,8 +505,11 @@ __device__ __forceinline__ SbTerms sb_terms_clamped(const Params& p, double sigm
 // error is below 2e-15 relative everywhere (what remains is the round-off of 8 FMAs).
 // mm_selftest_fastmath (include/mm_bench.h) measures it against the direct formulas.  Outside
 // [2^-5, 4) and for NaN the direct formulas are used.
+#ifndef MM_AB_SUBBITS
+#define MM_AB_SUBBITS 5
+#endif
 struct AbTable {
-    static constexpr int kSubBits = 5, kSub = 1 << kSubBits;        // sub-intervals per octave
+    static constexpr int kSubBits = MM_AB_SUBBITS, kSub = 1 << kSubBits;        // sub-intervals per octave
     static constexpr int kOctLo = -5, kOctaves = 7;                 // [2^-5, 2^2)
     static constexpr int kIntervals = kOctaves * kSub, kDeg = 8;
     static constexpr int kStride = 2 * (kDeg + 1);                  // (a_i, b_i) pairs, highest power first
