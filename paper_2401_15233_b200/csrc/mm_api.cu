@@ -29,7 +29,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
     int nm, pitch, rows;
-    size_t plane, state_bytes, off_ctrl, off_bc, off_tab, off_hist, off_u0, off_u1, total;
+    size_t plane, state_bytes, off_ctrl, off_bc, off_tab, off_hist, off_u0, off_u1, off_w0, off_w1, total;
 };
 
 bool make_layout(const mm_grid* g, Layout* L)
@@ -50,7 +50,10 @@ bool make_layout(const mm_grid* g, Layout* L)
     L->off_hist = L->off_tab + align_up(AbTable::kDoubles * sizeof(double), 256);
     L->off_u0 = L->off_hist + align_up((size_t)kDtHistory * sizeof(double), 256);
     L->off_u1 = L->off_u0 + L->state_bytes;
-    L->total = L->off_u1 + L->state_bytes;
+    // the 14-moment system keeps the primitives W(U) of both copies beside them (mm_tm14.cuh)
+    L->off_w0 = L->off_u1 + L->state_bytes;
+    L->off_w1 = L->off_w0 + (L->nm == 14 ? L->state_bytes : 0);
+    L->total = L->off_w1 + (L->nm == 14 ? L->state_bytes : 0);
     return true;
 }
 
@@ -82,6 +85,7 @@ struct mm_solver {
     Ctrl* ctrl;
     BcTable* bc;
     double* U[2];
+    double* W[2];       // 14-moment: primitives of U[0], U[1] (nullptr for the 5-moment system)
     int cur;            // buffer holding the current state
     int slot;           // accumulator slot holding the current state's CFL reduction
     int has_state;
@@ -114,8 +118,8 @@ int launch_ghost(mm_solver* s, const StepCtl& sc, int finalize)
 {
     const int n = 4 * s->p.ny + (NM == 5 ? 0 : 4 * s->p.nx);
     const int nt = 128, nb = (n + nt - 1) / nt;
-    k_ghost<NM><<<nb, nt, 0, s->stream>>>(s->p, s->U[s->cur], s->bc, s->ctrl, s->slot, sc, finalize,
-                                          (double*)(s->ws + s->L.off_hist));
+    k_ghost<NM><<<nb, nt, 0, s->stream>>>(s->p, NM == 14 ? s->W[s->cur] : s->U[s->cur], s->bc, s->ctrl, s->slot, sc,
+                                          finalize, (double*)(s->ws + s->L.off_hist), NM == 14);
     MM_LAUNCHED(s, "k_ghost");
     return MM_OK;
 }
@@ -134,7 +138,7 @@ int launch_pass(mm_solver* s, int in, int out, const double* base, double dt_sca
 #define MM_LAUNCH_TM(ZSV, EXTV)                                                                      \
     k_step14_tm<ZSV, EXTV><<<(items + Mom<ZSV>::NW - 1) / Mom<ZSV>::NW, 32 * Mom<ZSV>::NW,             \
                              Mom<ZSV>::smem_bytes, s->stream>>>(                                       \
-        s->p, s->U[in], s->U[out], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks[fast], base, dt_scale, do_rate)
+        s->p, s->W[in], s->U[in], s->W[out], s->U[out], s->ctrl, s->slot ^ 1, s->nstrips, s->nchunks[fast], base, dt_scale, do_rate)
         if (fast) { if (ext) MM_LAUNCH_TM(true, true); else MM_LAUNCH_TM(true, false); }
         else { if (ext) MM_LAUNCH_TM(false, true); else MM_LAUNCH_TM(false, false); }
 #undef MM_LAUNCH_TM
@@ -198,9 +202,18 @@ int set_state_impl(mm_solver* s, const double* src, int on_device, bool prim)
         dsrc = s->U[s->cur ^ 1];
     }
     dim3 grid((s->p.nx + 127) / 128, s->p.ny < 65535 ? s->p.ny : 65535);
-    if (prim) k_pack<NM, true><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur]);
-    else k_pack<NM, false><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur]);
+    if (prim) k_pack<NM, true><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur], s->W[s->cur]);
+    else k_pack<NM, false><<<grid, 128, 0, s->stream>>>(s->p, dsrc, s->U[s->cur], s->W[s->cur]);
     MM_LAUNCHED(s, "k_pack");
+    if constexpr (NM == 14) {
+        // the z-symmetric kernel variant leaves the z-odd planes alone: they are exact zeros in both copies
+        // (the idle copy may hold the staged input)
+        const int zodd[4] = {3, 6, 8, 12};
+        for (int m : zodd) {
+            MM_CUDA(cudaMemsetAsync(s->U[s->cur ^ 1] + (size_t)m * s->L.plane, 0, s->L.plane * sizeof(double), s->stream));
+            MM_CUDA(cudaMemsetAsync(s->W[s->cur ^ 1] + (size_t)m * s->L.plane, 0, s->L.plane * sizeof(double), s->stream));
+        }
+    }
     // reset the clock and the accumulators (keeps the constant ghost part)
     MM_CUDA(cudaMemsetAsync(s->ctrl, 0, offsetof(Ctrl, ghost_rate), s->stream));
     MM_CUDA(cudaMemsetAsync(&s->ctrl->steps, 0, sizeof(Ctrl) - offsetof(Ctrl, steps), s->stream));
@@ -232,8 +245,14 @@ int get_state_impl(mm_solver* s, double* dst, int on_device, bool prim)
     if (prim) k_unpack<NM, true><<<grid, 128, 0, s->stream>>>(s->p, s->U[s->cur], ddst);
     else k_unpack<NM, false><<<grid, 128, 0, s->stream>>>(s->p, s->U[s->cur], ddst);
     MM_LAUNCHED(s, "k_unpack");
-    if (!on_device)
+    if (!on_device) {
         MM_CUDA(cudaMemcpyAsync(dst, ddst, nbytes, cudaMemcpyDeviceToHost, s->stream));
+        if constexpr (NM == 14) {      // the idle copy served as staging: its z-odd planes are zeros again (see set_state_impl)
+            const int zodd[4] = {3, 6, 8, 12};
+            for (int m : zodd)
+                MM_CUDA(cudaMemsetAsync(s->U[s->cur ^ 1] + (size_t)m * s->L.plane, 0, s->L.plane * sizeof(double), s->stream));
+        }
+    }
     MM_CUDA(cudaStreamSynchronize(s->stream));
     return MM_OK;
 }
@@ -288,6 +307,8 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_gas* gas, const mm_
     s->bc = (BcTable*)(s->ws + L.off_bc);
     s->U[0] = (double*)(s->ws + L.off_u0);
     s->U[1] = (double*)(s->ws + L.off_u1);
+    s->W[0] = L.nm == 14 ? (double*)(s->ws + L.off_w0) : nullptr;
+    s->W[1] = L.nm == 14 ? (double*)(s->ws + L.off_w1) : nullptr;
     Params& p = s->p;
     p.sigma_lim = opt->sigma_lim; p.ws_scale = opt->ws_scale;
     p.dx = (grid->x1 - grid->x0) / grid->nx;

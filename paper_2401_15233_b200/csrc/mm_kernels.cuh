@@ -100,10 +100,22 @@ __device__ __forceinline__ void cell_rate(const Params& p, const double (&U)[NM]
     if (!ok || !(rate - rate == 0.0)) { bad = 1; rate = 0.0; speed = 0.0; }
 }
 
+// rate / speed / validity of one 14-moment cell from its primitives (the step kernel's tail holds them)
+template <class Z>
+__device__ __forceinline__ void prim_rate14(const Params& p, const double (&W)[14], double& rate,
+                                            double& speed, int& bad)
+{
+    double sx, sy;
+    const bool ok = cell_speeds14<Z>(p, W, sx, sy);
+    rate = dmax(sx / p.dx, sy / p.dy); speed = dmax(sx, sy);
+    if (!ok || !(rate - rate == 0.0)) { bad = 1; rate = 0.0; speed = 0.0; }
+}
+
 // ---------------------------------------------------------------- state in / out kernels
-// interior [NM][ny][nx] (conserved, or primitive when PRIM) -> padded conserved planes
+// interior [NM][ny][nx] (conserved, or primitive when PRIM) -> padded conserved planes `dst` and, for the
+// 14-moment system (dstW != nullptr), the padded primitive planes beside them (mm_tm14.cuh reads both)
 template <int NM, bool PRIM>
-__global__ void k_pack(Params p, const double* __restrict__ src, double* __restrict__ dst)
+__global__ void k_pack(Params p, const double* __restrict__ src, double* __restrict__ dst, double* __restrict__ dstW)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.nx) return;
@@ -120,6 +132,13 @@ __global__ void k_pack(Params p, const double* __restrict__ src, double* __restr
     }
 #pragma unroll
     for (int m = 0; m < NM; ++m) dst[m * plane + (size_t)(j + 2) * p.pitch + i + 2] = b[m];
+    if constexpr (NM == 14) {
+        if (dstW) {
+            if constexpr (!PRIM) cons2prim14<double>(b, a);      // a = W(U); given primitives are kept as they are
+#pragma unroll
+            for (int m = 0; m < NM; ++m) dstW[m * plane + (size_t)(j + 2) * p.pitch + i + 2] = a[m];
+        }
+    }
     }
 }
 
@@ -199,9 +218,12 @@ struct StepCtl {
 // Thread 0 also closes the CFL reduction of the state that is about to be stepped:
 // dt = cfl / max(rate, ghost_rate) (L434), advances t and the step counter, and clears the
 // accumulator slot the step kernel will max-reduce the NEXT state into.
+// `U` is the array the step kernel reconstructs from: the conserved planes of the 5-moment system, the
+// PRIMITIVE planes of the 14-moment system (prim = 1: Dirichlet cells take the table's W instead of its U;
+// the conserved planes of that system are only read at interior cells and need no ghost values).
 template <int NM>
 __global__ void k_ghost(Params p, double* __restrict__ U, const BcTable* __restrict__ tab,
-                        Ctrl* ctrl, int slot, StepCtl sc, int finalize, double* __restrict__ dt_hist)
+                        Ctrl* ctrl, int slot, StepCtl sc, int finalize, double* __restrict__ dt_hist, int prim)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (finalize && tid == 0) {
@@ -256,7 +278,7 @@ __global__ void k_ghost(Params p, double* __restrict__ U, const BcTable* __restr
         int k = b.has_default ? b.nbands : -1;
         for (int q = b.nbands - 1; q >= 0; --q)          // first matching band wins
             if (coord >= b.lo[q] && coord <= b.hi[q]) k = q;
-        if (k >= 0) fixed = b.U[k];
+        if (k >= 0) fixed = prim ? b.W[k] : b.U[k];
     }
 #pragma unroll
     for (int m = 0; m < NM; ++m) U[m * plane + gidx] = fixed ? fixed[m] : U[m * plane + sidx];
@@ -288,7 +310,7 @@ __global__ void __launch_bounds__(NT) k_rate(Params p, const double* __restrict_
 }
 
 // ------------------------------------------------------------------ the fused time step
-// (the 14-moment step kernel is in mm_strip14.cuh)
+// (the 14-moment step kernel is in mm_tm14.cuh)
 // 5-moment interface flux between cell a (low side) and cell b (high side) from the primitives
 // staged in shared memory.  `w` points at cell b of moment plane 0, `ms` is the plane stride.
 // MUSCL on primitives (L262-264): face states W_a + slope_a/2 and W_b - slope_b/2; closure flux,

@@ -16,10 +16,17 @@
 // that this tensor-core-free method would otherwise leave unused: registers hold one face, shared
 // memory only what lanes exchange (the primitives ring and the rows in flight).
 //
+// The state lives in HBM twice: the conserved moments U (what the update advances, Eq 16) and the
+// primitives W = W(U) (what the reconstruction reads, L264), both written by the tail of the step that
+// produced them -- the tail needs W(U^{n+1}) anyway for the CFL wave speeds (a9), so cons->prim runs
+// exactly once per cell and step, and no row is converted on load.  HBM has the bandwidth to spare
+// (this method runs at ~20 % of it), the FP64 pipe does not.
 // Per warp, in shared memory (NV = moments carried: 14, or the 10 z-even ones on the z-symmetric path):
-//   ring  [3][NV][34]  primitives of the rows r-1 .. r+1 (cells x0-2 .. x0+31), a ring over r;
-//   cons  [2][NV][34]  conserved rows in flight: filled by cp.async one row ahead of use, so the
-//                      HBM latency of row r+2 hides behind the work on row r at no register cost;
+//   ring  [3][NV][34]  primitives of the rows r-1 .. r+1 (cells x0-2 .. x0+31), a ring over r: row r+2
+//                      is copied by cp.async from W in HBM into the slot of row r-1 while the x
+//                      interfaces of row r are in work, at no register cost;
+//   own   [NV][32]     conserved moments of the lanes' own cells in row r+1 (the base of the update),
+//                      copied by cp.async in the same group;
 // per lane, in tensor memory (columns of 32 bit, 2 per double):
 //   face  [2 NV + 2]   F_k, U_k, lambda_min, lambda_max of the left face state of the interface in work;
 //   acc   [NV]         partial update of the lane's cell in the row being assembled;
@@ -59,18 +66,16 @@ struct Mom {
         return ZS ? t[m] : m;
     }
     __host__ __device__ static constexpr int cswap(int k) { return compact(swap_xy(full(k))); }
-    static constexpr int warp_smem_doubles = 3 * NV * kRW + 2 * NV * kRW;
+    static constexpr int warp_smem_doubles = 3 * NV * kRW + NV * 32;
 #ifndef MM_TM_NW_ZS
-#define MM_TM_NW_ZS 12
+#define MM_TM_NW_ZS 16
 #endif
 #ifndef MM_TM_NW_GEN
 #define MM_TM_NW_GEN 8
 #endif
     // Warps per block (one block per SM).  Registers are private to a scheduler (16384 each): 4 warps per
-    // scheduler leave 128 registers per thread, 3 leave 168, 2 leave 255.  Measured on the 2048^2 bench
-    // (z-symmetric variant): 16 warps x 128 registers (a few spills) 0.897 ms, 12 x 168 0.845 ms; the round-1
-    // kernel (two faces per thread, 8 x 240) 0.956 ms.  Shared memory: table 8.75 KB + NW x 13.3 KB
-    // (z-symmetric) resp. 18.6 KB (general).
+    // scheduler leave 128 registers per thread, 3 leave 168, 2 leave 255.  Shared memory: table 31.5 KB +
+    // NW x 10.5 KB (z-symmetric) resp. 14.7 KB (general).
     static constexpr int NW = ZS ? MM_TM_NW_ZS : MM_TM_NW_GEN;
     static constexpr size_t smem_bytes = ((size_t)AbTable::kDoubles + (size_t)NW * warp_smem_doubles) * sizeof(double) + 16;
     // tensor-memory columns of a lane: [face | acc | hsv]
@@ -133,8 +138,8 @@ __device__ __forceinline__ void tm_load(unsigned taddr, double (&v)[N])   // inc
 #endif
 template <bool ZS, bool EXT>
 __global__ void MM_TM_REGATTR
-k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl,
-            int slot_next, int nstrips, int nchunks, const double* Ubase_, double dt_scale_, int do_rate_)
+k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __restrict__ Uin, double* Wout, double* Uout,
+            Ctrl* ctrl, int slot_next, int nstrips, int nchunks, const double* Ubase_, double dt_scale_, int do_rate_)
 {
     const double* Ubase = EXT ? Ubase_ : nullptr;
     const double dt_scale = EXT ? dt_scale_ : 1.0;
@@ -161,7 +166,7 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const unsigned tm_base = *tm_slot;
     p.ab = smem;
-    // this warp's 32 lanes x 128 columns: lane quarter warp % 4 (the only one the warp may touch)
+    // this warp's 32 lanes x tm_stride columns: lane quarter warp % 4 (the only one the warp may touch)
     const unsigned tm = __shfl_sync(0xffffffffu, tm_base + ((unsigned)(32 * (warp & 3)) << 16)
                                                      + (unsigned)(M::tm_stride * (warp >> 2)), 0);
 
@@ -173,7 +178,7 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
     const int y1 = (int)((long long)(chunk + 1) * p.ny / nchunks);
     work = work && y1 > y0;
     double* ring = smem + AbTable::kDoubles + warp * M::warp_smem_doubles;
-    double* cons = ring + 3 * RS;
+    double* own = ring + 3 * RS;
     const size_t plane = (size_t)p.rows * p.pitch;
     const int ncell = min(kSW, p.nx - x0);            // cells of this strip
     const int ncol = min(kRW, p.nx + 4 - x0);         // staged columns that exist
@@ -184,20 +189,25 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
         if (cell_ok)
             for (int r = y0; r < y1; ++r)
 #pragma unroll
-                for (int m = 0; m < NM; ++m)
-                    Uout[m * plane + (size_t)(r + 2) * p.pitch + ccol] = Uin[m * plane + (size_t)(r + 2) * p.pitch + ccol];
+                for (int m = 0; m < NM; ++m) {
+                    if (ZS && z_odd(m)) continue;
+                    const size_t o = m * plane + (size_t)(r + 2) * p.pitch + ccol;
+                    Uout[o] = Uin[o]; Wout[o] = Win[o];
+                }
         work = false;
     }
     if (work) {
-    // U_out = B - dt div F(U_in) + source:  B = U_in for forward Euler and for the half step of the
+    // U_out = B - dt div F(W_in) + source:  B = U_in for forward Euler and for the half step of the
     // midpoint scheme (dt_scale = 1/2, no CFL reduction); B = Ubase = U^n for its full step, which
     // may be written in place (Uout == Ubase: a cell's B is read by the lane that later writes it).
     const double dt = ctrl->dt * dt_scale;
     const double dtdx = dt / p.dx, dtdy = dt / p.dy;
+    const int cl = min(max(lane, 1), ncell) + 1;     // y: ring column of the lane's cell (clamped to valid cells)
+    const int cx = min(lane, ncol - 3);              // x: ring column of cell M (= cell C - 1), clamped
 
-    auto load_row = [&](int r, int cslot) {          // interior row r in [-2, ny+1] -> cons[cslot]
-        const double* src = Uin + (size_t)(r + 2) * p.pitch + x0;
-        double* dst = cons + cslot * RS;
+    auto load_row = [&](int r, int rslot) {          // primitives of interior row r in [-2, ny+1] -> ring[rslot]
+        const double* src = Win + (size_t)(r + 2) * p.pitch + x0;
+        double* dst = ring + rslot * RS;
         if (lane < ncol) {
 #pragma unroll
             for (int k = 0; k < NV; ++k) cp_async8(dst + k * kRW + lane, src + M::full(k) * plane + lane);
@@ -206,38 +216,23 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
 #pragma unroll
             for (int k = 0; k < NV; ++k) cp_async8(dst + k * kRW + 32 + lane, src + M::full(k) * plane + 32 + lane);
         }
-        cp_async_commit();
     };
-    auto convert_row = [&](int cslot, int rslot) {   // cons[cslot] -> primitives in ring[rslot] (a2)
-        const double* src = cons + cslot * RS;
-        double* dst = ring + rslot * RS;
-#pragma unroll 1
-        for (int c = lane; c < ncol; c += 32) {
-            double U[NM], W[NM];
+    auto load_own = [&](int r) {                     // conserved moments of the lanes' own cells in row r -> own
+        if (!Ubase) {
+            const double* src = Uin + (size_t)(r + 2) * p.pitch + x0 + cl;
 #pragma unroll
-            for (int k = 0; k < NV; ++k) U[M::full(k)] = src[k * kRW + c];
-            cons2prim14<Z>(U, W);
-#pragma unroll
-            for (int k = 0; k < NV; ++k) dst[k * kRW + c] = W[M::full(k)];
+            for (int k = 0; k < NV; ++k) cp_async8(own + k * 32 + lane, src + M::full(k) * plane);
         }
     };
 
-    load_row(y0 - 2, 0); load_row(y0 - 1, 1);
+    load_row(y0 - 2, 0); load_row(y0 - 1, 1); load_row(y0, 2);
+    cp_async_commit();
     cp_async_wait_all(); __syncwarp();
-    convert_row(0, 0); convert_row(1, 1);
-    __syncwarp();
-    load_row(y0, 0); load_row(y0 + 1, 1);            // stay in cons: U of rows y0, y0+1
-    cp_async_wait_all(); __syncwarp();
-    convert_row(0, 2);
-    __syncwarp();
     int sm = 0, sc = 1, sp = 2;                      // ring slots of the rows r-1, r, r+1
 
     double rate = 0.0, speed = 0.0;
     int bad = 0;
-    const int cl = min(max(lane, 1), ncell) + 1;     // y: ring column of the lane's cell (clamped to valid cells)
-    const int cx = min(lane, ncol - 3);              // x: ring column of cell M (= cell C - 1), clamped
     for (int r = y0 - 1; r <= y1; ++r) {
-        const int cs = (r - y0) & 1;
 #pragma unroll 1
         for (int d = 0; d < 2; ++d) {
             // Lanes without an interface of their own (beyond the strip's last cell / staged column)
@@ -248,9 +243,13 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
                 const double* b = ring + cl;
                 qm = b + sm * RS; qc = b + sc * RS; qp = b + sp * RS;
             } else {                                 // x: C = (row r, cell lane-1), M = cell lane-2
-                if (r < y0 || r == y1) break;
-                __syncwarp();                        // every lane has taken U_r out of cons[cs]
-                load_row(r + 2, cs);
+                if (r == y1) break;
+                // row r-1 and the own cells of row r are done with: rows r+2 / r+1 into their places
+                __syncwarp();
+                load_row(r + 2, sm);
+                if (r + 1 < y1) load_own(r + 1);
+                cp_async_commit();
+                if (r < y0) break;
                 qm = ring + sc * RS + cx; qc = qm + 1; qp = qm + 2;
             }
             // ---- a3: limited half slope of C; face states of the interface M|C
@@ -347,16 +346,19 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
                             add_source14<Z>(W, dt * inv_tau(p, W[0], (W[4] + W[7] + W[9]) * (1.0 / 3.0)), Un);
                         }
                     }
+                    // the primitives of the new state (a2 of the next step) and its CFL wave speeds (a9)
+                    double Wn[NM];
+                    cons2prim14<Z>(Un, Wn);
                     if (cell_ok) {
-                        double* out = Uout + (size_t)(r + 1) * p.pitch + ccol;
+                        const size_t o = (size_t)(r + 1) * p.pitch + ccol;
 #pragma unroll
-                        for (int m = 0; m < NM; ++m) {
-                            if (ZS && z_odd(m)) out[m * plane] = 0.0;
-                            else out[m * plane] = Un[m];
+                        for (int k = 0; k < NV; ++k) {
+                            Uout[M::full(k) * plane + o] = Un[M::full(k)];
+                            Wout[M::full(k) * plane + o] = Wn[M::full(k)];
                         }
                         if (do_rate) {
                             double rr, ss;
-                            cell_rate<NM, Z>(p, Un, rr, ss, bad);
+                            prim_rate14<Z>(p, Wn, rr, ss, bad);
                             rate = dmax(rate, rr); speed = dmax(speed, ss);
                         }
                     }
@@ -368,7 +370,7 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
                         for (int k = 0; k < NV; ++k) A[k] = __dadd_rn(ub[M::full(k) * plane], __dmul_rn(dtdy, G[k]));
                     } else {
 #pragma unroll
-                        for (int k = 0; k < NV; ++k) A[k] = __dadd_rn(cons[cs * RS + k * kRW + cl], __dmul_rn(dtdy, G[k]));
+                        for (int k = 0; k < NV; ++k) A[k] = __dadd_rn(own[k * 32 + lane], __dmul_rn(dtdy, G[k]));
                     }
                     tm_store<NV>(tm + M::tm_acc, A);
                 }
@@ -384,10 +386,8 @@ k_step14_tm(const Params pg, const double* __restrict__ Uin, double* Uout, Ctrl*
                 tm_store<NV>(tm + M::tm_acc, A);
             }
         }
-        if (r < y1) {                                // row r+2 has landed: primitives into the slot of row r-1
+        if (r < y1) {                                // rows r+2 (primitives) and r+1 (own cells) have landed
             cp_async_wait_all(); __syncwarp();
-            convert_row(cs, sm);
-            __syncwarp();
             const int t = sm; sm = sc; sc = sp; sp = t;
         }
     }

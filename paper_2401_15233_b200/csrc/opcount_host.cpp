@@ -2,8 +2,10 @@
 // update (the "algorithmic flops" of the roofline line).
 // mm_physics.cuh is compiled on the HOST with `double` replaced by a counting type; the
 // composition below mirrors what the fused step kernel does for ONE cell with no tile overhead:
-//   1 cons->prim, per direction 1 limited slope and 1 interface (2 face evaluations, HLL),
-//   the update, the BGK source and the tail CFL evaluation of the new state.
+//   per direction 1 limited slope and 1 interface (2 face evaluations, HLL), the update, the BGK
+//   source, and the tail: cons->prim of the new state and its CFL wave speeds.  The 14-moment kernel
+//   reads the primitives the previous step's tail stored (one cons->prim per cell and step); the
+//   5-moment kernel converts on load as well.
 // Convention: each + - * / sqrt exp pow = 1 (an FMA is 2); comparisons, fabs,
 // fmin/fmax, negation and copies = 0.  The wave-speed functions a(P*), b(P*) are booked as the method's
 // formulas (10 operations per call), not as the table evaluation the kernel executes.  Measurement tooling only; nothing here is linked into libmm.so.
@@ -115,7 +117,8 @@ static long long one_cell(Params p, int ndim)
     if constexpr (NM == 5) prim2cons5(W[1], U); else prim2cons14<Z>(W[1], U);
     half_slope<NM>(p, W[0], W[1], W[2], hm, zs);       // the neighbour's slope (its own cost)
     cnt::ops = 0;
-    if constexpr (NM == 5) cons2prim5(U, Wc); else cons2prim14<Z>(U, Wc);
+    if constexpr (NM == 5) cons2prim5(U, Wc);
+    else for (int k = 0; k < NM; ++k) Wc[k] = W[1][k];     // stored by the previous step's tail (mm_tm14.cuh)
     const cnt dt = 1e-3, dtdx = dt / p.dx, dtdy = dt / p.dy;
     for (int d = 0; d < ndim; ++d) {          // each cell owns one slope and one interface per direction
         half_slope<NM>(p, W[1], W[2], W[3], hc, zs);

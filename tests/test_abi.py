@@ -63,8 +63,8 @@ def test_binding_structs_match_header(mm):
 def test_workspace_bytes_and_argument_checks(mm):
     lib = mm.lib()
     n = mm.mm_workspace_bytes(14, 2048, 2048)
-    # two padded state copies of 14 planes dominate
-    planes = 2 * 14 * (2048 + 4) * 2064 * 8
+    # two padded state copies of 14 planes, each as conserved moments and as primitives, dominate
+    planes = 4 * 14 * (2048 + 4) * 2064 * 8
     assert planes <= n <= planes + 600000         # + control block, boundary tables, a/b table, dt history
     assert mm.mm_workspace_bytes(5, 1000, 1) > 2 * 5 * 1004 * 5 * 8
     assert mm.mm_workspace_bytes(5, 10, 2) == 0          # 1-D system needs ny = 1
@@ -130,7 +130,7 @@ def test_launch_decomposition_host_logic(mm):
             if nx * ny >= 512 * 512:
                 ideal = ns * (ny + 0.8 * nc) / slots
                 assert waves * (rows + 0.8) <= (1.15 if nx * ny >= 1024 * 1024 else 1.2) * ideal
-    assert mm.mm_decomposition(2048, 2048, True, 148)[::2] == (69, 12)
+    assert mm.mm_decomposition(2048, 2048, True, 148)[::2] == (69, 16)
     with pytest.raises(mm.MMError):
         mm.mm_decomposition(0, 5)
 
