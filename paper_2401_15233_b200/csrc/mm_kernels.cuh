@@ -107,7 +107,7 @@ __device__ __forceinline__ void prim_rate14(const Params& p, const double (&W)[1
 {
     double sx, sy;
     const bool ok = cell_speeds14<Z>(p, W, sx, sy);
-    rate = dmax(sx / p.dx, sy / p.dy); speed = dmax(sx, sy);
+    rate = dmax(sx * p.inv_dx, sy * p.inv_dy); speed = dmax(sx, sy);
     if (!ok || !(rate - rate == 0.0)) { bad = 1; rate = 0.0; speed = 0.0; }
 }
 

@@ -43,6 +43,25 @@ __host__ __device__ __forceinline__ void zput(double&, zero_t) {}
 __host__ __device__ __forceinline__ void zadd(double& dst, const double& v) { dst = dst + v; }
 __host__ __device__ __forceinline__ void zadd(double&, zero_t) {}
 
+// a * b + c as ONE explicitly fused operation, with the exact-zero type folded away.  Routines written with
+// it produce the same bits in every kernel and instantiation they are inlined into (the compiler's own
+// contraction of a * b + c depends on the surrounding code): cons2prim14 needs that, because the primitives
+// mm_set_state derives from a checkpointed U must equal the ones the step kernel's tail derived from it.
+template <class T> struct is_zero_t : std::false_type {};
+template <> struct is_zero_t<zero_t> : std::true_type {};
+template <class A, class B, class C>
+__device__ __forceinline__ auto ffma(const A& a, const B& b, const C& c)
+{
+    if constexpr (is_zero_t<A>::value || is_zero_t<B>::value) return c;
+#ifdef MM_OPCOUNT_HOST
+    else if constexpr (is_zero_t<C>::value) return a * b;
+    else return a * b + c;
+#else
+    else if constexpr (is_zero_t<C>::value) return __dmul_rn(a, b);
+    else return fma(a, b, c);
+#endif
+}
+
 // ------------------------------------------------------------------ reciprocal / square root
 // rcp(x) ~ 1/x and fsqrt(x) ~ sqrt(x) to ~1 ulp for normal x: hardware seed (MUFU.RCP64H /
 // MUFU.RSQ64H, ~20 bits) + one higher-order Newton step, branch-free (no slow-path call).
@@ -130,6 +149,7 @@ struct Params {               // per-solver constants, passed by value to the ke
     double sigma_lim;         // L163, L512
     double ws_scale;          // k of L409
     double dx, dy, x0, y0;
+    double inv_dx, inv_dy;    // 1/dx, 1/dy (CFL rate of a cell without a division)
     double inv_tau_coef;      // MM_TAU_KN: 1/tau = inv_tau_coef * rho * sqrt(8 P /(pi rho))
     double inv_tau_const;     // MM_TAU_CONST: 1/tau
     double R_gas;             // T = P/(rho R_gas): Maxwellian Dirichlet states (k_bc_table)
@@ -356,24 +376,30 @@ __device__ __forceinline__ void numflux(int flux, const double (&FL)[NM], const 
 template <class Z>
 __device__ __forceinline__ void cons2prim14(const double (&U)[14], double (&W)[14])
 {
+    // written with the momenta m_i = rho u_i and the trace U_jj = rho u^2 + P_jj of the conserved state itself:
+    //   P_ij = U_ij - m_i u_j,   q_i = U_ijj - u_i U_jj - 2 P_ij u_j,
+    //   R = U_iijj - u^2 (U_jj + P_jj) - 4 u_i (P_ij u_j + q_i)
+    // every multiply-add is an explicit ffma (bit-reproducible across kernels, see ffma)
     const double rho = U[0], ir = rcp(rho);
-    const double ux = U[1] * ir, uy = U[2] * ir;
-    const Z uz = zget<Z>(U[3]) * ir;
-    const double Pxx = U[4] - rho * ux * ux, Pxy = U[5] - rho * ux * uy;
-    const Z Pxz = zget<Z>(U[6]) - rho * ux * uz;
-    const double Pyy = U[7] - rho * uy * uy;
-    const Z Pyz = zget<Z>(U[8]) - rho * uy * uz;
-    const double Pzz = U[9] - rho * uz * uz;
-    const double u2 = ux * ux + uy * uy + uz * uz, trP = Pxx + Pyy + Pzz;
-    const double Pux = Pxx * ux + Pxy * uy + Pxz * uz;
-    const double Puy = Pxy * ux + Pyy * uy + Pyz * uz;
-    const Z Puz = Pxz * ux + Pyz * uy + Pzz * uz;
-    const double e = rho * u2 + trP;
-    const double qx = U[10] - ux * e - 2.0 * Pux;
-    const double qy = U[11] - uy * e - 2.0 * Puy;
-    const Z qz = zget<Z>(U[12]) - uz * e - 2.0 * Puz;
-    const double uPu = ux * Pux + uy * Puy + uz * Puz, uq = ux * qx + uy * qy + uz * qz;
-    const double R = U[13] - rho * u2 * u2 - 2.0 * u2 * trP - 4.0 * uPu - 4.0 * uq;
+    const double mx = U[1], my = U[2];
+    const Z mz = zget<Z>(U[3]);
+    const double ux = mx * ir, uy = my * ir;
+    const Z uz = mz * ir;
+    const double Pxx = ffma(-mx, ux, U[4]), Pxy = ffma(-mx, uy, U[5]);
+    const Z Pxz = ffma(-mx, uz, zget<Z>(U[6]));
+    const double Pyy = ffma(-my, uy, U[7]);
+    const Z Pyz = ffma(-my, uz, zget<Z>(U[8]));
+    const double Pzz = ffma(-mz, uz, U[9]);
+    const double e = (U[4] + U[7]) + U[9], trP = (Pxx + Pyy) + Pzz;
+    const double Pux = ffma(Pxz, uz, ffma(Pxy, uy, Pxx * ux));
+    const double Puy = ffma(Pyz, uz, ffma(Pyy, uy, Pxy * ux));
+    const Z Puz = ffma(Pzz, uz, ffma(Pyz, uy, Pxz * ux));
+    const double qx = ffma(-2.0, Pux, ffma(-ux, e, U[10]));
+    const double qy = ffma(-2.0, Puy, ffma(-uy, e, U[11]));
+    const Z qz = ffma(-2.0, Puz, ffma(-uz, e, zget<Z>(U[12])));
+    const double u2 = ffma(uz, uz, ffma(uy, uy, ux * ux));
+    const double uPq = ffma(uz, Puz + qz, ffma(uy, Puy + qy, ux * (Pux + qx)));
+    const double R = ffma(-4.0, uPq, ffma(-u2, e + trP, U[13]));
     W[0] = rho; W[1] = ux; W[2] = uy; zput(W[3], uz);
     W[4] = Pxx; W[5] = Pxy; zput(W[6], Pxz); W[7] = Pyy; zput(W[8], Pyz); W[9] = Pzz;
     W[10] = qx; W[11] = qy; zput(W[12], qz); W[13] = R;
@@ -396,12 +422,13 @@ __device__ __forceinline__ void prim2cons14(const double (&W)[14], double (&U)[1
     U[0] = rho; U[1] = rux; U[2] = ruy; zput(U[3], ruz);
     U[4] = rux * ux + Pxx; U[5] = rux * uy + Pxy; zput(U[6], rux * uz + Pxz);
     U[7] = ruy * uy + Pyy; zput(U[8], ruy * uz + Pyz); U[9] = ruz * uz + Pzz;
-    U[10] = ux * e + 2.0 * Pux + W[10];
-    U[11] = uy * e + 2.0 * Puy + W[11];
-    zput(U[12], uz * e + 2.0 * Puz + qz);
-    const double uPu = ux * Pux + uy * Puy + uz * Puz;
-    const double uq = ux * W[10] + uy * W[11] + uz * qz;
-    U[13] = rho * u2 * u2 + 2.0 * u2 * trP + 4.0 * uPu + 4.0 * uq + W[13];
+    const double qx = W[10], qy = W[11];
+    U[10] = ux * e + (2.0 * Pux + qx);
+    U[11] = uy * e + (2.0 * Puy + qy);
+    zput(U[12], uz * e + (2.0 * Puz + qz));
+    // rho u^4 + 2 u^2 P_jj + 4 u_i u_j P_ij + 4 u_i q_i + R, factored
+    const double uPq = ux * (Pux + qx) + uy * (Puy + qy) + uz * (Puz + qz);
+    U[13] = u2 * (rho * u2 + 2.0 * trP) + (4.0 * uPq + W[13]);
 }
 
 // Dimensionless state (Eq 6, rho* = 1): c = sqrt(P/rho), P = P_ii/3, p = P_ij/P (tr p = 3),
@@ -420,18 +447,19 @@ struct Star14 {
 };
 
 template <class Z>
-__device__ __forceinline__ void nondim_sigma14(const double (&W)[14], Star14<Z>& s)
+__device__ __forceinline__ void nondim_sigma14(const Params& p, const double (&W)[14], Star14<Z>& s)
 {
     const double rho = W[0];
-    const double Ph = (W[4] + W[7] + W[9]) * (1.0 / 3.0);
-    const double rr = rcp(Ph * rho), iP = rr * rho, ir = rr * Ph;      // one reciprocal for both
-    const double c2 = Ph * ir, c = fsqrt_pos(c2);
+    const double Ph = (W[4] + W[7] + W[9]) * p.k13;
+    // one reciprocal square root serves c, 1/P and 1/(rho c^3):  y = (P rho)^-1/2, c = P y, 1/P = rho y^2
+    const double y = rsqrt_nr(Ph * rho), ry = rho * y, iP = ry * y;
+    const double c = Ph * y;
     s.c = c; s.Ph = Ph;
     s.pxx = W[4] * iP; s.pxy = W[5] * iP; s.pxz = zget<Z>(W[6]) * iP;
     s.pyy = W[7] * iP; s.pyz = zget<Z>(W[8]) * iP; s.pzz = W[9] * iP;
-    const double ih = iP * (c * rho * iP);                 // 1/(rho c^3) = 1/(P c)
+    const double ih = iP * ry;                             // 1/(rho c^3) = 1/(P c) = rho y / P
     s.hx = W[10] * ih; s.hy = W[11] * ih; s.hz = zget<Z>(W[12]) * ih;
-    const double Rs = W[13] * rho * iP * iP;               // R/(rho c^4) = R rho / P^2
+    const double Rs = W[13] * (rho * iP) * iP;             // R/(rho c^4) = R rho / P^2
     s.sxx = s.pxx * s.pxx + s.pxy * s.pxy + s.pxz * s.pxz;
     s.sxy = s.pxx * s.pxy + s.pxy * s.pyy + s.pxz * s.pyz;
     s.sxz = s.pxx * s.pxz + s.pxy * s.pyz + s.pxz * s.pzz;
@@ -659,7 +687,7 @@ template <class Z, bool TABLE_ONLY = false>
 __device__ __forceinline__ void eval_face14_A(const Params& p, const double (&W)[14], FaceA<Z>& a,
                                               double& lmin, double& lmax)
 {
-    nondim_sigma14<Z>(W, a.s);
+    nondim_sigma14<Z>(p, W, a.s);
     a.t = sb_terms_clamped(p, a.s.sigma);
     wavespeed14_x<Z, TABLE_ONLY>(p, a.s, a.t, W[1], lmin, lmax);
 }
@@ -678,12 +706,12 @@ __device__ __forceinline__ void eval_face14_B(const Params& p, const double (&W)
     const SbTerms& t = fa.t;
     const double sb = t.sb, isb = t.isb, ss = t.ss;
 
-    const double I2 = 0.5 * (9.0 - s.t2), I3 = s.I3;
-    const double t3 = 3.0 * s.t2 - 3.0 * I2 + 3.0 * I3;
-    // B = 12 p^2 + (2 t2 - 4 I2) p + 4 I3 I
-    const double bp = 2.0 * s.t2 - 4.0 * I2, b0 = 4.0 * I3;
-    const double Bxx = 12.0 * s.sxx + bp * s.pxx + b0, Bxy = 12.0 * s.sxy + bp * s.pxy;
-    const double Byy = 12.0 * s.syy + bp * s.pyy + b0;
+    // Cayley-Hamilton coefficients with I1 = tr p = 3, I2 = (9 - t2)/2, t3 = 3 t2 - 3 I2 + 3 I3 substituted:
+    //   B = 12 p^2 + (4 t2 - 18) p + 4 I3 I,   M = (24 t2 + 216) p^2 + (108 t2 - 648 + 56 I3) p + 120 I3 I
+    const double I3 = s.I3;
+    const double bp = 4.0 * s.t2 - 18.0, b0 = 4.0 * I3;
+    const double Bxx = 12.0 * s.sxx + (bp * s.pxx + b0), Bxy = 12.0 * s.sxy + bp * s.pxy;
+    const double Byy = 12.0 * s.syy + (bp * s.pyy + b0);
     double vx, vy;
     Z vz;
     if constexpr (std::is_same<Z, zero_t>::value) {
@@ -692,7 +720,7 @@ __device__ __forceinline__ void eval_face14_B(const Params& p, const double (&W)
         vy = (Bxx * s.hy - Bxy * s.hx) * idB;
     } else {
         const double Bxz = 12.0 * s.sxz + bp * s.pxz, Byz = 12.0 * s.syz + bp * s.pyz;
-        const double Bzz = 12.0 * s.szz + bp * s.pzz + b0;
+        const double Bzz = 12.0 * s.szz + (bp * s.pzz + b0);
         const double cxx = Byy * Bzz - Byz * Byz, cxy = Bxz * Byz - Bxy * Bzz;
         const double cxz = Bxy * Byz - Bxz * Byy, cyy = Bxx * Bzz - Bxz * Bxz;
         const double cyz = Bxy * Bxz - Bxx * Byz, czz = Bxx * Byy - Bxy * Bxy;
@@ -704,34 +732,33 @@ __device__ __forceinline__ void eval_face14_B(const Params& p, const double (&W)
     const double ax = s.pxx * vx + s.pxy * vy + s.pxz * vz;
     const double ay = s.pxy * vx + s.pyy * vy + s.pyz * vz;
     const Z az = s.pxz * vx + s.pyz * vy + s.pzz * vz;
-    // Q*_ijx
-    const double Qxx = 6.0 * ax * s.sxx;
-    const double Qxy = 2.0 * (2.0 * ax * s.sxy + ay * s.sxx);
-    const Z Qxz = 2.0 * (2.0 * ax * s.sxz + az * s.sxx);
-    const double Qyy = 2.0 * (2.0 * ay * s.sxy + ax * s.syy);
-    const Z Qyz = 2.0 * (ay * s.sxz + ax * s.syz + az * s.sxy);
-    const double Qzz = 2.0 * (2.0 * az * s.sxz + ax * s.szz);
-    // T_i = Q*_ixl w_l
-    const double Tx = Qxx * s.wx + Qxy * s.wy + Qxz * s.wz;
-    const double Ty = Qxy * s.wx + Qyy * s.wy + Qyz * s.wz;
-    const Z Tz = Qxz * s.wx + Qyz * s.wy + Qzz * s.wz;
-    const double g = 2.0 * (1.0 - sb);
-    const double Rxs = Tx * isb + g * s.sxx + 3.0 * s.pxx;
-    const double Rys = Ty * isb + g * s.sxy + 3.0 * s.pxy;
-    const Z Rzs = Tz * isb + g * s.sxz + 3.0 * s.pxz;
-    const double m2 = 14.0 * s.t2 + 306.0 - 20.0 * I2;
-    const double m1 = 54.0 - 6.0 * s.t2 + 12.0 * t3 - 120.0 * I2 + 20.0 * I3;
+    // dimensional Q_ijx = rho c^3 Q*_ijx, the scale folded into a: A = 2 rho c^3 a  (rho c^2 = P)
+    const double rc3 = s.Ph * s.c, rc4 = rc3 * s.c, rc5 = rc4 * s.c, k2 = 2.0 * rc3;
+    const double Ax = k2 * ax, Ay = k2 * ay;
+    const Z Az = k2 * az;
+    const double Qxxx = 3.0 * (Ax * s.sxx);
+    const double Qxyx = 2.0 * (Ax * s.sxy) + Ay * s.sxx;
+    const Z Qxzx = 2.0 * (Ax * s.sxz) + Az * s.sxx;
+    const double Qyyx = 2.0 * (Ay * s.sxy) + Ax * s.syy;
+    const Z Qyzx = Ay * s.sxz + Ax * s.syz + Az * s.sxy;
+    const double Qzzx = 2.0 * (Az * s.sxz) + Ax * s.szz;
+    // T_i = Q_ixl w_l (dimensional: rho c^3 T*)
+    const double Tx = Qxxx * s.wx + Qxyx * s.wy + Qxzx * s.wz;
+    const double Ty = Qxyx * s.wx + Qyyx * s.wy + Qyzx * s.wz;
+    const Z Tz = Qxzx * s.wx + Qyzx * s.wy + Qzzx * s.wz;
+    // R_ix = rho c^4 R*_ix = (c / sb) T_i + rho c^4 [2 (1 - sb) (p^2)_ix + 3 p_ix]                    (Eq 23)
+    const double g = 2.0 - 2.0 * sb, ci = s.c * isb;
+    const double Rx = ci * Tx + rc4 * (g * s.sxx + 3.0 * s.pxx);
+    const double Ry = ci * Ty + rc4 * (g * s.sxy + 3.0 * s.pxy);
+    const Z Rz = ci * Tz + rc4 * (g * s.sxz + 3.0 * s.pxz);
+    // S_x = rho c^5 S*_x = (c / sb)^2 (w . T) + rho c^5 [6 sqrt(sb) h_x + (1 - sqrt(sb)) (M v)_x]    (Eq 24)
+    const double m2 = 24.0 * s.t2 + 216.0;
+    const double m1 = 108.0 * s.t2 + (56.0 * I3 - 648.0);
     const double m0 = 120.0 * I3;
     const double pax = s.pxx * ax + s.pxy * ay + s.pxz * az;          // (p^2 v)_x
-    const double Mvx = m2 * pax + m1 * ax + m0 * vx;
-    const double Sxs = (s.wx * Tx + s.wy * Ty + s.wz * Tz) * (isb * isb) + 6.0 * ss * s.hx
-                     + (1.0 - ss) * Mvx;
-    // re-dimensionalise: Q = rho c^3 Q*, R = rho c^4 R*, S = rho c^5 S*  (rho c^2 = P)
-    const double rc3 = s.Ph * s.c, rc4 = rc3 * s.c, rc5 = rc4 * s.c;
-    const double Qxxx = rc3 * Qxx, Qxyx = rc3 * Qxy, Qyyx = rc3 * Qyy, Qzzx = rc3 * Qzz;
-    const Z Qxzx = rc3 * Qxz, Qyzx = rc3 * Qyz;
-    const double Rx = rc4 * Rxs, Ry = rc4 * Rys, Sx = rc5 * Sxs;
-    const Z Rz = rc4 * Rzs;
+    const double Mvx = m2 * pax + (m1 * ax + m0 * vx);
+    const double Sx = (ci * ci) * (s.wx * Tx + s.wy * Ty + s.wz * Tz)
+                    + rc5 * ((6.0 * ss) * s.hx + (1.0 - ss) * Mvx);
 
     prim2cons14<Z>(W, U);
     const double ux = W[1], uy = W[2];
@@ -742,23 +769,24 @@ __device__ __forceinline__ void eval_face14_B(const Params& p, const double (&W)
     const double u2 = ux * ux + uy * uy + uz * uz;
     const double uPx = ux * Pxx + uy * Pxy + uz * Pxz;                 // u_j P_jx
     F[0] = U[1];                                                       // 16a
-    F[1] = ux * U[1] + Pxx;                                            // 16b
-    F[2] = ux * U[2] + Pxy;
-    zput(F[3], ux * zget<Z>(U[3]) + Pxz);
-    F[4] = ux * U[4] + 2.0 * ux * Pxx + Qxxx;                          // 16c
-    F[5] = ux * U[5] + ux * Pxy + uy * Pxx + Qxyx;
-    zput(F[6], ux * zget<Z>(U[6]) + ux * Pxz + uz * Pxx + Qxzx);
-    F[7] = ux * U[7] + 2.0 * uy * Pxy + Qyyx;
-    zput(F[8], ux * zget<Z>(U[8]) + uy * Pxz + uz * Pxy + Qyzx);
-    F[9] = ux * U[9] + 2.0 * uz * Pxz + Qzzx;
+    F[1] = U[4];                                                       // 16b: rho u_i u_x + P_ix = U_ix
+    F[2] = U[5];
+    zput(F[3], zget<Z>(U[6]));
+    F[4] = ux * (U[4] + 2.0 * Pxx) + Qxxx;                             // 16c
+    F[5] = ux * (U[5] + Pxy) + (uy * Pxx + Qxyx);
+    zput(F[6], ux * (zget<Z>(U[6]) + Pxz) + (uz * Pxx + Qxzx));
+    F[7] = ux * U[7] + ((2.0 * uy) * Pxy + Qyyx);
+    zput(F[8], ux * zget<Z>(U[8]) + (uy * Pxz + uz * Pxy + Qyzx));
+    F[9] = ux * U[9] + ((2.0 * uz) * Pxz + Qzzx);
     const double k1 = 2.0 * uPx + qx;                                  // 16d
-    F[10] = ux * U[10] + ux * k1 + u2 * Pxx + 2.0 * (ux * Qxxx + uy * Qxyx + uz * Qxzx) + Rx;
-    F[11] = ux * U[11] + uy * k1 + u2 * Pxy + 2.0 * (ux * Qxyx + uy * Qyyx + uz * Qyzx) + Ry;
-    zput(F[12], ux * zget<Z>(U[12]) + uz * k1 + u2 * Pxz + 2.0 * (ux * Qxzx + uy * Qyzx + uz * Qzzx) + Rz);
-    const double uuQ = ux * (ux * Qxxx + 2.0 * (uy * Qxyx + uz * Qxzx))
-                     + uy * (uy * Qyyx + 2.0 * uz * Qyzx) + uz * uz * Qzzx;
-    F[13] = ux * U[13] + 2.0 * u2 * k1 + 4.0 * (uuQ + ux * Rx + uy * Ry + uz * Rz) + Sx;   // 16e
-
+    const double uQx = ux * Qxxx + uy * Qxyx + uz * Qxzx;              // u_j Q_jix
+    const double uQy = ux * Qxyx + uy * Qyyx + uz * Qyzx;
+    const Z uQz = ux * Qxzx + uy * Qyzx + uz * Qzzx;
+    F[10] = ux * (U[10] + k1) + (u2 * Pxx + (2.0 * uQx + Rx));
+    F[11] = ux * U[11] + (uy * k1 + (u2 * Pxy + (2.0 * uQy + Ry)));
+    zput(F[12], ux * zget<Z>(U[12]) + (uz * k1 + (u2 * Pxz + (2.0 * uQz + Rz))));
+    // 16e: u_x U_iijj + 2 u^2 (2 u_j P_jx + q_x) + 4 u_i (u_j Q_ijx + R_ix) + S_x
+    F[13] = ux * U[13] + ((2.0 * u2) * k1 + (4.0 * (ux * (uQx + Rx) + uy * (uQy + Ry) + uz * (uQz + Rz)) + Sx));
 }
 
 template <class Z>
@@ -767,8 +795,17 @@ __device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[1
                                             double& lmax)
 {
     FaceA<Z> a;
+#ifndef MM_OPCOUNT_HOST
+    // a(P*), b(P*) straight from the table: no branch between the wave-speed chains of part A and the
+    // multiply-add-rich part B, so the two interleave; the (rare) state outside the table's range redoes
+    // its wave speeds with the direct formulas afterwards
+    eval_face14_A<Z, true>(p, W, a, lmin, lmax);
+    eval_face14_B<Z>(p, W, a, F, U);
+    if (!ab_in_table(a.s.pxx)) face14_speeds_direct<Z>(p, W, a, lmin, lmax);
+#else
     eval_face14_A<Z>(p, W, a, lmin, lmax);
     eval_face14_B<Z>(p, W, a, F, U);
+#endif
 }
 
 // max(|lmin|,|lmax|) along x and y of a cell-centre state, for the CFL reduction (L434).
@@ -780,7 +817,7 @@ __device__ __forceinline__ bool cell_speeds14(const Params& p, const double (&W)
     double Ph = W[4] + W[7] + W[9];
     if (!(W[0] > 0.0) || !(Ph > 0.0)) { sx = sy = 0.0; return false; }
     Star14<Z> s;
-    nondim_sigma14<Z>(W, s);
+    nondim_sigma14<Z>(p, W, s);
     const SbTerms t = sb_terms_clamped(p, s.sigma);
     double a, b;
     wavespeed14_x<Z>(p, s, t, W[1], a, b);
