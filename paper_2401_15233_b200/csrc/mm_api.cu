@@ -369,13 +369,7 @@ int mm_create(mm_solver** out, const mm_grid* grid, const mm_gas* gas, const mm_
     s->allow_fast = 1;
     if (nm == 14) {
         k_ab_table<<<AbTable::kIntervals, 2, 0, s->stream>>>((double*)(s->ws + L.off_tab));
-        k_sb_lim<<<1, 1, 0, s->stream>>>(p.sigma_lim, s->ctrl);
-        s->launches += 2;
-        double lim[4];
-        e = cudaMemcpyAsync(lim, s->ctrl->sb_lim, sizeof lim, cudaMemcpyDeviceToHost, s->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
-        if (e != cudaSuccess) { delete s; return cuda_fail(e, "k_sb_lim"); }
-        p.lim_ss = lim[0]; p.lim_isb = lim[1]; p.lim_B = lim[2]; p.lim_sqB = lim[3];
+        s->launches += 1;
         e = cudaFuncSetAttribute(k_step14_tm<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(k_step14_tm<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGen);

@@ -20,7 +20,6 @@ struct Ctrl {
     double ghost_rate, ghost_speed;                   // constant part from Dirichlet ghost states
     long long bc_bad;                                 // a Dirichlet state has rho <= 0 or P <= 0
     long long bc_znz;                                 // a Dirichlet state has a non-zero z-odd moment
-    double sb_lim[4];                                 // sb_terms(sigma_lim): ss, isb, B, sqB (k_sb_lim, read back at create)
     long long steps;
     int bad[2];                                       // reduction saw rho<=0, P<=0 or non-finite
     int failed;                                       // sticky: stepping stopped (MM_ENONFINITE)
@@ -315,6 +314,20 @@ __global__ void __launch_bounds__(NT) k_rate(Params p, const double* __restrict_
 // staged in shared memory.  `w` points at cell b of moment plane 0, `ms` is the plane stride.
 // MUSCL on primitives (L262-264): face states W_a + slope_a/2 and W_b - slope_b/2; closure flux,
 // conserved state and wave speeds of both (eval_face5), then HLL / Rusanov.
+// psi/4 of the cells a and b of the stencil (am, a, b, bp) with the shared limiter (L266)
+template <int LIM>
+__device__ __forceinline__ void shared_psi_pair5(const double (&Wam)[5], const double (&Wa)[5], const double (&Wb)[5],
+                                                 const double (&Wbp)[5], double& qa, double& qb)
+{
+    PsiShared<LIM> ma, mb;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        ma.add(Wa[k] - Wam[k], Wb[k] - Wa[k], (Wa[k] - Wam[k]) + (Wb[k] - Wa[k]));
+        mb.add(Wb[k] - Wa[k], Wbp[k] - Wb[k], (Wb[k] - Wa[k]) + (Wbp[k] - Wb[k]));
+    }
+    qa = 0.25 * ma.psi(); qb = 0.25 * mb.psi();
+}
+
 __device__ __forceinline__ void interface_flux5(const Params& p, const double* __restrict__ w,
                                                 int ms, double (&Fh)[5])
 {
@@ -326,13 +339,9 @@ __device__ __forceinline__ void interface_flux5(const Params& p, const double* _
         Wam[k] = q[-2]; Wa[k] = q[-1]; Wb[k] = q[0]; Wbp[k] = q[1];
     }
     if (p.limiter != 0 && p.shared_limiter) {
-        PsiShared ma, mb;
-#pragma unroll
-        for (int k = 0; k < NM; ++k) {
-            ma.add(p.limiter, Wa[k] - Wam[k], Wb[k] - Wa[k], (Wa[k] - Wam[k]) + (Wb[k] - Wa[k]));
-            mb.add(p.limiter, Wb[k] - Wa[k], Wbp[k] - Wb[k], (Wb[k] - Wa[k]) + (Wbp[k] - Wb[k]));
-        }
-        const double qa = 0.25 * ma.psi(), qb = 0.25 * mb.psi();
+        double qa, qb;
+        if (p.limiter == 1) shared_psi_pair5<1>(Wam, Wa, Wb, Wbp, qa, qb);
+        else shared_psi_pair5<2>(Wam, Wa, Wb, Wbp, qa, qb);
 #pragma unroll
         for (int k = 0; k < NM; ++k) {
             WL[k] = Wa[k] + qa * ((Wa[k] - Wam[k]) + (Wb[k] - Wa[k]));
@@ -420,13 +429,6 @@ k_step5(Params p, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl, int 
         if (do_rate) cell_rate<NM>(p, Un, rate, speed, bad);
     }
     if (do_rate) block_reduce_rate<NT>(rate, speed, bad, ctrl, slot_next);
-}
-
-// sb_terms(sigma_lim) for Params::lim_* (one thread, at mm_create)
-__global__ void k_sb_lim(double sigma_lim, Ctrl* ctrl)
-{
-    const SbTerms t = sb_terms(sigma_lim);
-    ctrl->sb_lim[0] = t.ss; ctrl->sb_lim[1] = t.isb; ctrl->sb_lim[2] = t.B; ctrl->sb_lim[3] = t.sqB;
 }
 
 // cos(pi n / d) for integers n >= 0, d > 0, reduced exactly to the first quadrant so that the

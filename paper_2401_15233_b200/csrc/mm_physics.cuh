@@ -160,9 +160,6 @@ struct Params {               // per-solver constants, passed by value to the ke
     // Literals whose low word is not zero (0.8, 0.1, ... of Eq 29, 1/3) cost two register moves per use
     // as immediates; as kernel parameters they are constant-bank operands of the FP64 instructions.
     double k08, k01, k06, k038, k035, k13;
-    // sb_terms(sigma_lim), evaluated once on the device at mm_create (k_sb_lim): a warp whose lanes all sit at
-    // sigma_bar = sigma_lim (every near-equilibrium region) takes these instead of three square roots per state
-    double lim_ss, lim_isb, lim_B, lim_sqB;
     __host__ void set_constants() { k08 = 0.8; k01 = 0.1; k06 = 0.6; k038 = 0.38; k035 = 0.35; k13 = 1.0 / 3.0; }
 };
 
@@ -192,12 +189,15 @@ __device__ __forceinline__ double limited_slope(int lim, double dm, double dp)
 // a variable with dm = dp = 0 has N = D = 0 and never wins the comparison, i.e. imposes nothing
 // (R14).  The running maximum is kept as a fraction and compared by cross-multiplication;
 // one reciprocal per slope forms psi.  `s` = dm + dp is shared with the slope itself.
+// LIM (1 minmod, 2 van Albada) is a template parameter: a run-time test inside the unrolled loop over the
+// variables is if-converted by the compiler into BOTH formulas plus a select per variable.
+template <int LIM>
 struct PsiShared {
     double n = 0.0, d = 1.0;
-    __device__ __forceinline__ void add(int lim, double dm, double dp, double s)
+    __device__ __forceinline__ void add(double dm, double dp, double s)
     {
         double nk, dk;
-        if (lim == 1) { nk = fabs(dm - dp); dk = fabs(s); }
+        if (LIM == 1) { nk = fabs(dm - dp); dk = fabs(s); }
         else { const double t = dm - dp; nk = t * t; dk = dm * dm + dp * dp; }
         if (nk * d > n * dk) { n = nk; d = dk; }
     }
@@ -209,6 +209,22 @@ struct PsiShared {
     }
 };
 
+template <int LIM, int NV>
+__device__ __forceinline__ void shared_half_slopes(const double (&Wm)[NV], const double (&Wc)[NV],
+                                                   const double (&Wp)[NV], double (&h)[NV])
+{
+    PsiShared<LIM> pm;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        const double dm = Wc[k] - Wm[k], dp = Wp[k] - Wc[k];
+        h[k] = dm + dp;
+        pm.add(dm, dp, h[k]);
+    }
+    const double q = 0.25 * pm.psi();
+#pragma unroll
+    for (int k = 0; k < NV; ++k) h[k] = q * h[k];
+}
+
 // a3: limited HALF slopes h_k of one cell along one direction from the primitives of its two neighbours
 // (L262-266): h = psi (dm + dp)/4 with one shared psi (L266), or h_k = limited_slope_k / 2 per variable.
 template <int NV>
@@ -219,16 +235,8 @@ __device__ __forceinline__ void half_slopes(const Params& p, const double (&Wm)[
 #pragma unroll
         for (int k = 0; k < NV; ++k) h[k] = 0.0;
     } else if (p.shared_limiter) {
-        PsiShared pm;
-#pragma unroll
-        for (int k = 0; k < NV; ++k) {
-            const double dm = Wc[k] - Wm[k], dp = Wp[k] - Wc[k];
-            h[k] = dm + dp;
-            pm.add(p.limiter, dm, dp, h[k]);
-        }
-        const double q = 0.25 * pm.psi();
-#pragma unroll
-        for (int k = 0; k < NV; ++k) h[k] = q * h[k];
+        if (p.limiter == 1) shared_half_slopes<1, NV>(Wm, Wc, Wp, h);
+        else shared_half_slopes<2, NV>(Wm, Wc, Wp, h);
     } else {
 #pragma unroll
         for (int k = 0; k < NV; ++k) h[k] = 0.5 * limited_slope(p.limiter, Wc[k] - Wm[k], Wp[k] - Wc[k]);
@@ -507,19 +515,12 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
     t.sqB = fsqrt_pos(t.B);
     return t;
 }
-// sigma_bar = clamp(sigma) and its terms.  When every active lane of the warp is limited to sigma_lim the
-// terms are the constants sb_terms(sigma_lim) held in Params (bit-identical: same routine, same device).
+// sigma_bar = clamp(sigma) and its terms.  (A warp-uniform shortcut for sigma_bar = sigma_lim -- the terms are
+// constants there -- was measured and dropped: the branch splits the face evaluation into two basic blocks,
+// which costs 1.5 % on near-equilibrium and on developed jet states alike, more than the skipped square roots save.)
 __device__ __forceinline__ SbTerms sb_terms_clamped(const Params& p, double sigma)
 {
-    const double sb = clamp_sigma(sigma, p.sigma_lim);
-#ifndef MM_OPCOUNT_HOST
-    if (__all_sync(__activemask(), sb == p.sigma_lim)) {
-        SbTerms t;
-        t.sb = sb; t.ss = p.lim_ss; t.isb = p.lim_isb; t.B = p.lim_B; t.sqB = p.lim_sqB;
-        return t;
-    }
-#endif
-    return sb_terms(sb);
+    return sb_terms(clamp_sigma(sigma, p.sigma_lim));
 }
 
 // ---- a(P*) = 1.4 P*^1.1 exp(-P*^2) and b(P*) = 0.9 P* exp(-P*^1.4 / 2) of Eq 29c-d (L397-399)
@@ -631,7 +632,7 @@ __device__ __forceinline__ void ws14_dir(const Params& p, double Pdd, double hd,
     const double cst = 4.0 * t.sb * t.sb * (sY * sY) + p.k01 * qt2;
     const double alpha = (p.k06 * Pdd - p.k038) * Pdd + p.k035;      // Eq 29b
     const double zp = hd + alpha * qt, zm = -hd + alpha * qt;        // Eq 30: q_d -> -q_d
-    const double rp = dmax(zp * zp - zp * sC + cst, kTiny), rm = dmax(zm * zm - zm * sC + cst, kTiny);
+    const double rp = dmax(zp * (zp - sC) + cst, kTiny), rm = dmax(zm * (zm - sC) + cst, kTiny);
     lam_max = pref * (zp + fsqrt_pos(rp)) + E;
     lam_min_neg = pref * (zm + fsqrt_pos(rm)) + E;
 }

@@ -283,7 +283,7 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
             // ---- a4-a7: the two face states through the closure, one after the other; the left face's
             // results wait in tensor memory
             double F[NM], U[NM], lmin, lmax;
-#pragma unroll 1
+#pragma unroll 1          // one copy of the face evaluation (two copies: 0.74 instead of 0.69 ms, instruction cache)
             for (int side = 0; side < 2; ++side) {
                 eval_face14<Z>(p, Wf, F, U, lmin, lmax);
                 if (side == 0) {

@@ -57,12 +57,12 @@ template <int NM>
 static void half_slope(const Params& p, const cnt (&Wm)[NM], const cnt (&Wc)[NM], const cnt (&Wp)[NM],
                        cnt (&h)[NM], bool zs)
 {
-    PsiShared pm;
+    PsiShared<1> pm;                                   // counted for minmod (p.limiter = 1 in main)
     for (int k = 0; k < NM; ++k) {
         if (NM == 14 && zs && z_odd(k)) continue;
         const cnt dm = Wc[k] - Wm[k], dp = Wp[k] - Wc[k];
         h[k] = dm + dp;
-        if (p.shared_limiter) pm.add(p.limiter, dm, dp, h[k]);
+        if (p.shared_limiter) pm.add(dm, dp, h[k]);
         else h[k] = 0.5 * limited_slope(p.limiter, dm, dp);
     }
     if (p.shared_limiter) {
