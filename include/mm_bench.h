@@ -19,6 +19,14 @@ extern "C" {
  * from the kernel's own clock64() / globaltimer readings (MHz). */
 int mm_measure_fp64_peak(void *stream, int repeats, double *tflops, double *sm_mhz);
 
+/* Instruction rates of the FP64 pipe with operands the register-reuse cache cannot supply (the same launch shape
+ * as mm_measure_fp64_peak; every instruction reads distinct registers of a 16-value ring), in 10^12 thread
+ * instructions per second:  tinstr[0] DFMA d = fma(a, b, d) with three distinct registers, [1] DMUL, [2] DADD.
+ * On B200 the DFMA of mm_measure_fp64_peak (multiplier and addend loop-invariant) and DMUL / DADD issue every 2
+ * cycles per scheduler, a DFMA with three distinct register operands every 3: the realistic ceiling of code that is
+ * not a polynomial in one variable. */
+int mm_measure_fp64_operand_rates(void *stream, int repeats, double tinstr[3]);
+
 /* Accuracy of the library's own elementary functions, measured on `stream` over n pseudo-random
  * arguments: max relative error in units of 2^-53 of
  * max_ulp[0] the branch-free reciprocal and [1] square root against IEEE (1e-30 .. 1e30),

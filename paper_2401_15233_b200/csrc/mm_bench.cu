@@ -32,6 +32,30 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, doubl
     if (threadIdx.x == 0) { out[1 + 2 * blockIdx.x] = (double)(c1 - c0); out[2 + 2 * blockIdx.x] = (double)(n1 - n0); }
 }
 
+// The same loop with operands the register-reuse cache cannot supply: every instruction reads distinct
+// registers of a 16-value ring.  MODE 0: d = fma(a, b, d) (three registers); 1: d = a * b; 2: d = a + b.
+// Values stay bounded (|x| ~ 1e-3 decays or saturates; no overflow, no denormal slow path on this pipe).
+template <int MODE>
+__global__ void __launch_bounds__(256) k_fp64_distinct(double* out, int iters)
+{
+    double x[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) x[k] = 0.5 + (double)(threadIdx.x + 7 * k) * 1e-4;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const int j = (k + 5) & 15, l = (k + 11) & 15;
+            if (MODE == 0) x[k] = fma(x[j], x[l], -x[k]);
+            else if (MODE == 1) x[k] = x[j] * x[l];
+            else x[k] = x[j] - x[l];
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s += x[k];
+    if (s == 123.456) out[0] = s;
+}
+
 // max relative error (in units of 2^-53) of rcp / fsqrt against IEEE 1/x and sqrt(x), and of the
 // tabulated a(P*), b(P*) against the direct formulas on (0, 3]
 __global__ void k_fastmath_test(int n, unsigned long long* err_bits, const double* __restrict__ tab)
@@ -101,6 +125,39 @@ int mm_measure_fp64_peak(void* stream, int repeats, double* tflops, double* sm_m
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out); delete[] h_out;
     *tflops = best;
     if (sm_mhz) *sm_mhz = mhz;
+    return rc;
+}
+
+int mm_measure_fp64_operand_rates(void* stream, int repeats, double* ginstr)
+{
+    if (!ginstr || repeats < 1) return -1;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
+    const int iters = 10000, blocks = sms * 8, threads = 256;
+    double* d_out = nullptr;
+    if (cudaMalloc(&d_out, sizeof(double)) != cudaSuccess) return -3;             // measurement scratch only
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    int rc = 0;
+    for (int mode = 0; mode < 3 && rc == 0; ++mode) {
+        double best = 0.0;
+        for (int r = 0; r < repeats + 1; ++r) {
+            cudaEventRecord(e0, st);
+            if (mode == 0) k_fp64_distinct<0><<<blocks, threads, 0, st>>>(d_out, iters);
+            else if (mode == 1) k_fp64_distinct<1><<<blocks, threads, 0, st>>>(d_out, iters);
+            else k_fp64_distinct<2><<<blocks, threads, 0, st>>>(d_out, iters);
+            cudaEventRecord(e1, st);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = -3; break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            const double g = 16.0 * (double)iters * blocks * threads / (ms * 1e-3) * 1e-12;   // 10^12 thread instructions / s
+            if (r > 0 && g > best) best = g;
+        }
+        ginstr[mode] = best;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
     return rc;
 }
 

@@ -279,8 +279,12 @@ __global__ void k_ghost(Params p, double* __restrict__ U, const BcTable* __restr
             if (coord >= b.lo[q] && coord <= b.hi[q]) k = q;
         if (k >= 0) fixed = prim ? b.W[k] : b.U[k];
     }
+    // all loads first: a store through U may alias the next load, which would chain NM memory round trips
+    double v[NM];
 #pragma unroll
-    for (int m = 0; m < NM; ++m) U[m * plane + gidx] = fixed ? fixed[m] : U[m * plane + sidx];
+    for (int m = 0; m < NM; ++m) v[m] = fixed ? fixed[m] : U[m * plane + sidx];
+#pragma unroll
+    for (int m = 0; m < NM; ++m) U[m * plane + gidx] = v[m];
 }
 
 // Standalone CFL reduction over the interior (used after mm_set_state).

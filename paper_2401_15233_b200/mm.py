@@ -32,7 +32,7 @@ EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim
            "mm_batch5_workspace_bytes", "mm_batch5_create", "mm_batch5_set_state_prim", "mm_batch5_step",
            "mm_batch5_step_fixed_dt", "mm_batch5_advance_to", "mm_batch5_get_state", "mm_batch5_get_info",
            "mm_batch5_launch_count", "mm_batch5_destroy"]
-BENCH_EXPORTS = ["mm_measure_fp64_peak", "mm_selftest_fastmath"]          # include/mm_bench.h, libmm_bench.so
+BENCH_EXPORTS = ["mm_measure_fp64_peak", "mm_measure_fp64_operand_rates", "mm_selftest_fastmath"]          # include/mm_bench.h, libmm_bench.so
 
 _dp = C.POINTER(C.c_double)
 
@@ -131,6 +131,7 @@ def bench_lib() -> C.CDLL:
         vp, i = C.c_void_p, C.c_int
         B.mm_measure_fp64_peak.restype, B.mm_measure_fp64_peak.argtypes = i, [vp, i, _dp, _dp]
         B.mm_selftest_fastmath.restype, B.mm_selftest_fastmath.argtypes = i, [vp, i, _dp]
+        B.mm_measure_fp64_operand_rates.restype, B.mm_measure_fp64_operand_rates.argtypes = i, [vp, i, _dp]
         _bench_lib = B
     return _bench_lib
 
@@ -160,6 +161,16 @@ def mm_measure_fp64_peak(repeats: int = 5, stream=None, with_clock: bool = False
     tf, mhz = C.c_double(), C.c_double()
     _check(bench_lib().mm_measure_fp64_peak(C.c_void_p(st.cuda_stream), repeats, C.byref(tf), C.byref(mhz)))
     return (tf.value, mhz.value) if with_clock else tf.value
+
+
+def mm_measure_fp64_operand_rates(repeats: int = 3, stream=None):
+    """10^12 thread instructions / s of the FP64 pipe with operands the reuse cache cannot supply:
+    (DFMA with three distinct registers, DMUL, DADD); include/mm_bench.h."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    out = (C.c_double * 3)()
+    _check(bench_lib().mm_measure_fp64_operand_rates(C.c_void_p(st.cuda_stream), repeats, out))
+    return tuple(out)
 
 
 def mm_decomposition(nx: int, ny: int, zsym: bool = True, sms: int = 148):
