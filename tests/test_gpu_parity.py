@@ -587,12 +587,47 @@ def test_batch5_matches_independent_oracle_tubes(mm, mmo):
     for j, t in enumerate(tubes):
         t.advance_to(0.03, 0.5)
         assert inf["t"][j] == 0.03
-        # step counts are themselves round-off sensitive at small sigma_lim (an oracle run perturbed by
-        # 1e-15 changes its own count by ~10 %, cf. test_C1_roundoff_sensitivity): a loose band only
-        assert abs(int(inf["steps"][j]) - t.info()["steps"]) <= 0.3 * t.info()["steps"]
+        # (the step COUNT of a single run is chaotic at small sigma_lim and is compared as a distribution,
+        # test_batch5_step_count_distribution_matches_the_oracle)
         rho_o = t.get_state()[0, 0]
         assert np.abs(Ub[j, 0] - rho_o).mean() <= 5e-3 * rho_o.mean()
     assert len(set(inf["steps"].tolist())) > 1
+
+
+def test_batch5_step_count_distribution_matches_the_oracle(mm, mmo):
+    """The number of CFL steps to t_end (the paper's cost measure, L342) is round-off chaotic at small sigma_lim:
+    24 oracle runs of the SAME tube (sigma_lim 1e-4, Kn 0.01, 333 cells, t_end 0.03) whose initial states differ by
+    1e-15 relative need between ~770 and ~1210 steps (measured, R24), so one GPU count against one
+    oracle count says nothing.  The batch runs the same 24 states as 24 tubes: the two count distributions must
+    agree -- medians within 12 %, quartiles within 20 %, every tube inside the oracle's range widened by its own
+    spread -- and every tube lands on t_end."""
+    nx, sl, kn, ne = 333, 1e-4, 0.01, 24
+    prob = wl.sod5(nx, Kn=kn, sigma_lim=sl)
+    Ws = []
+    for seed in range(ne):
+        W = prob["W0"].copy()
+        if seed:
+            W *= 1.0 + 1e-15 * np.random.default_rng(seed).standard_normal(W.shape)
+        Ws.append(W.reshape(5, nx))
+    b = mm.Batch5(nx, [sl] * ne, [kn] * ne)
+    b.set_state_prim(np.stack(Ws))
+    b.advance_to(0.03, 0.5)
+    inf = b.info()
+    assert np.all(inf["t"] == 0.03)
+    g = np.sort(inf["steps"].astype(float))
+    o = []
+    for W in Ws:
+        so = oracle_solver(mmo, prob)
+        so.set_state_prim(W.reshape(5, 1, nx))
+        so.advance_to(0.03, 0.5)
+        o.append(so.info()["steps"])
+    o = np.sort(np.array(o, dtype=float))
+    assert o.max() > 1.2 * o.min()                               # the premise: the count is chaotic in the oracle itself
+    assert abs(np.median(g) - np.median(o)) <= 0.12 * np.median(o), (g, o)
+    for qt in (0.25, 0.75):
+        assert abs(np.quantile(g, qt) - np.quantile(o, qt)) <= 0.20 * np.quantile(o, qt), (g, o)
+    spread = o.max() - o.min()
+    assert g.min() >= o.min() - spread and g.max() <= o.max() + spread, (g, o)
 
 
 def test_batch5_cost_rises_as_sigma_lim_falls(mm):
