@@ -597,7 +597,7 @@ bool batch_layout(int nx, int ntubes, BLayout* L)
 int batch_step(mm_batch5* b, const StepCtl& sc)
 {
     k_batch5_finalize<<<(b->ntubes + 127) / 128, 128, 0, b->stream>>>(b->ntubes, b->ctl, b->slot, sc);
-    dim3 grid((b->nx + kNTB - 1) / kNTB, b->ntubes);
+    dim3 grid((b->nx + kNTB - 2) / (kNTB - 1), b->ntubes);       // kNTB - 1 cells per block (mm_batch5.cuh)
     k_batch5_step<kNTB><<<grid, kNTB, 0, b->stream>>>(b->p, b->sigma_lim, b->inv_tau_coef, b->U[b->cur],
                                                      b->U[b->cur ^ 1], b->ctl, b->slot ^ 1);
     b->launches += 2;

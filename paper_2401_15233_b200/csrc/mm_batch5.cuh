@@ -9,6 +9,10 @@
 #pragma once
 #include "mm_kernels.cuh"
 
+#ifndef MM_BATCH5_MINB
+#define MM_BATCH5_MINB 8        // resident blocks of 128 threads per SM the step kernel is compiled for
+#endif
+
 namespace mm {
 
 struct TubeCtl {                       // one per tube, device memory
@@ -99,19 +103,22 @@ k_batch5_rate(Params p, const double* __restrict__ sigma_lim, const double* __re
 }
 
 // One step of every tube.  State layout: [tube][moment][nx], no ghost storage.
+// A block of NT threads owns NT - 1 cells: thread t evaluates the interface on the LEFT of cell gx0 + t
+// (t = 0 .. NT-1, one per thread -- an (NT+1)-th interface would be a second pass of warp 0 alone, with every
+// other warp waiting at the barrier), threads 0 .. NT-2 update their cells.
 template <int NT>
-__global__ void __launch_bounds__(NT)
+__global__ void __launch_bounds__(NT, MM_BATCH5_MINB)
 k_batch5_step(Params p, const double* __restrict__ sigma_lim, const double* __restrict__ inv_tau_coef,
               const double* __restrict__ Uin, double* __restrict__ Uout, TubeCtl* ctl, int slot_next)
 {
-    constexpr int NM = 5, PW = NT + 4, PF = NT + 1;
+    constexpr int NM = 5, NC = NT - 1, PW = NT + 3, PF = NT;
     __shared__ double Ws[NM * PW];
     __shared__ double Fx[NM * PF];
-    const int j = blockIdx.y, tid = threadIdx.x, gx0 = blockIdx.x * NT;
+    const int j = blockIdx.y, tid = threadIdx.x, gx0 = blockIdx.x * NC;
     const size_t off = (size_t)j * NM * p.nx;
     const double* uin = Uin + off;
     double* uout = Uout + off;
-    const bool cell_ok = gx0 + tid < p.nx;
+    const bool cell_ok = tid < NC && gx0 + tid < p.nx;
     TubeCtl* c = &ctl[j];
     if (c->skip) {
         if (cell_ok)
@@ -121,7 +128,7 @@ k_batch5_step(Params p, const double* __restrict__ sigma_lim, const double* __re
     }
     const Params q = tube_params(p, sigma_lim, inv_tau_coef, j);
     const double dt = c->dt;
-    // stage cells gx0-2 .. gx0+NT+1; beyond the ends the boundary cell is repeated (L426, zero gradient)
+    // stage cells gx0-2 .. gx0+NT; beyond the ends the boundary cell is repeated (L426, zero gradient)
     for (int idx = tid; idx < PW; idx += NT) {
         const int i = min(max(gx0 + idx - 2, 0), p.nx - 1);
         double U[NM], W[NM];
@@ -132,18 +139,17 @@ k_batch5_step(Params p, const double* __restrict__ sigma_lim, const double* __re
         for (int m = 0; m < NM; ++m) Ws[m * PW + idx] = W[m];
     }
     __syncthreads();
-    for (int idx = tid; idx < PF; idx += NT) {
-        if (gx0 + idx > p.nx) continue;
+    if (gx0 + tid <= p.nx) {
         double Fh[NM];
-        interface_flux5(q, Ws + idx + 2, PW, Fh);
+        interface_flux5(q, Ws + tid + 2, PW, Fh);
 #pragma unroll
-        for (int m = 0; m < NM; ++m) Fx[m * PF + idx] = Fh[m];
+        for (int m = 0; m < NM; ++m) Fx[m * PF + tid] = Fh[m];
     }
     __syncthreads();
     double rate = 0.0, speed;
     int bad = 0;
     if (cell_ok) {
-        const double dtdx = dt / p.dx;
+        const double dtdx = dt * p.inv_dx;
         double Un[NM], W[NM];
 #pragma unroll
         for (int m = 0; m < NM; ++m) {

@@ -88,12 +88,12 @@ __device__ __forceinline__ void cell_rate(const Params& p, const double (&U)[NM]
         cons2prim5(U, W);
         double sx;
         ok = cell_speed5(p, W, sx);
-        rate = sx / p.dx; speed = sx;
+        rate = sx * p.inv_dx; speed = sx;
     } else {
         cons2prim14<Z>(U, W);
         double sx, sy;
         ok = cell_speeds14<Z>(p, W, sx, sy);
-        rate = dmax(sx / p.dx, sy / p.dy); speed = dmax(sx, sy);
+        rate = dmax(sx * p.inv_dx, sy * p.inv_dy); speed = dmax(sx, sy);
     }
     // finite test: NaN or Inf fail (x - x != 0)
     if (!ok || !(rate - rate == 0.0)) { bad = 1; rate = 0.0; speed = 0.0; }
@@ -411,7 +411,7 @@ k_step5(Params p, const double* __restrict__ Uin, double* Uout, Ctrl* ctrl, int 
     double rate = 0.0, speed = 0.0;
     int bad = 0;
     if (cell_ok) {
-        const double dtdx = dt / p.dx;
+        const double dtdx = dt * p.inv_dx;
         double Un[NM], W[NM];
 #pragma unroll
         for (int m = 0; m < NM; ++m) {

@@ -296,8 +296,9 @@ __device__ __forceinline__ void wavespeed5(const Params& p, const double (&W)[5]
                                            double& lmax)
 {
     double rho = W[0], u = W[1], P = W[2], q = W[3], r = W[4];
-    double c2 = P * rcp(rho), c = fsqrt_pos(c2);
-    double irc4 = rcp(rho * c2 * c2);                     // 1/(rho c^4); 1/(rho c^3) = c/(rho c^4)
+    // one reciprocal square root: y = (P rho)^-1/2, c = P y, 1/P = rho y^2, 1/(rho c^4) = rho / P^2
+    double y = rsqrt_nr(P * rho), c = P * y, iP = (rho * y) * y;
+    double irc4 = (rho * iP) * iP;                        // 1/(rho c^4); 1/(rho c^3) = c/(rho c^4)
     double qs = q * (c * irc4), rs = r * irc4;
     double sb = clamp_sigma(sigma5(qs, rs), p.sigma_lim);
     WS5 w = ws5_common(sb);
@@ -310,9 +311,9 @@ __device__ __forceinline__ void eval_face5(const Params& p, const double (&W)[5]
                                            double (&U)[5], double& lmin, double& lmax)
 {
     double rho = W[0], u = W[1], P = W[2], q = W[3], r = W[4];
-    double c2 = P * rcp(rho), c = fsqrt_pos(c2);
-    double rc3 = rho * c2 * c;
-    double irc4 = rcp(rc3 * c);
+    double y = rsqrt_nr(P * rho), c = P * y, iP = (rho * y) * y;     // as in wavespeed5
+    double c2 = c * c, rc3 = P * c;                                  // rho c^2 = P
+    double irc4 = (rho * iP) * iP;
     double qs = q * (c * irc4), rs = r * irc4;
     double sb = clamp_sigma(sigma5(qs, rs), p.sigma_lim);
     // Eq 15 (L155): s* = q*^3/sigma^2 + (10 - 8 sqrt(sigma)) q*;  s = rho c^5 s*

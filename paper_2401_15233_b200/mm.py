@@ -196,6 +196,7 @@ class Solver:
     `bcs`: 4 dicts (xlo, xhi, ylo, yhi): {"type": BC_*, "bands": [(lo, hi, W), ...], "default": W|None,
     "state": STATE_PRIMITIVE (W = nmom primitives) | STATE_MAXWELLIAN (W = (rho, u_x, u_y, u_z, T))}.
     `R_gas`: mm_gas.R_gas (T = P/(rho R_gas); only Maxwellian boundary states use it).
+    `workspace`: optional CUDA uint8 tensor of >= mm_workspace_bytes + 255 bytes to use instead of a fresh one.
     State arrays are [nmom][ny][nx]; numpy arrays / CPU tensors go through the host path
     (on_device = 0), CUDA tensors through the device path (on_device = 1)."""
 
@@ -203,7 +204,8 @@ class Solver:
                  collision: Optional[dict] = None, bcs: Optional[Sequence[dict]] = None,
                  sigma_lim: float = 1e-4, ws_scale: float = 1.0, limiter: int = LIM_MINMOD,
                  shared_limiter: int = 0, flux: int = FLUX_HLL, source_scheme: int = SRC_EXPLICIT,
-                 time_scheme: int = TIME_EULER, R_gas: float = 1.0, device: str = "cuda:0", stream=None):
+                 time_scheme: int = TIME_EULER, R_gas: float = 1.0, device: str = "cuda:0", stream=None,
+                 workspace=None):
         import torch
         if not torch.cuda.is_available():
             raise MMError(ECUDA, "no CUDA device: the moment-method library has no CPU path")
@@ -236,7 +238,11 @@ class Solver:
                            bw.ctypes.data_as(_dp), dw.ctypes.data_as(_dp) if dw is not None else None, kind)
         with torch.cuda.device(self.device):
             self._stream = stream if stream is not None else torch.cuda.current_stream()
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            if workspace is None:
+                workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            elif workspace.dtype != torch.uint8 or not workspace.is_cuda or workspace.numel() < nbytes + 255:
+                raise MMError(EWORKSPACE, f"workspace must be a CUDA uint8 tensor of at least {nbytes + 255} bytes")
+            self.workspace = workspace          # caller-owned device memory (mm.h): the library allocates none
             base = self.workspace.data_ptr()
             self._ws_ptr = (base + 255) // 256 * 256
             o = mm_options(sigma_lim, ws_scale, limiter, shared_limiter, flux, source_scheme, time_scheme,
