@@ -135,6 +135,19 @@ static const double kTiny = 0x1p-996;
 #else
 constexpr double kTiny = 0x1p-996;
 #endif
+// max(x, kTiny) for the floored radicands (R6), decided on the high word with integer instructions: for x >= kTiny
+// (and for NaN, which passes through) the signed high word is >= that of kTiny; negative, zero and subnormal x have
+// a smaller one.  Same values as dmax(x, kTiny), without an FP64-pipe compare.
+#ifdef MM_OPCOUNT_HOST
+__forceinline__ double floor_tiny(double x) { return dmax(x, kTiny); }
+#else
+__device__ __forceinline__ double floor_tiny(double x)
+{
+    const int hi = __double2hiint(x);
+    const bool ok = hi >= 0x01b00000;                      // high word of 2^-996
+    return __hiloint2double(ok ? hi : 0x01b00000, ok ? __double2loint(x) : 0);
+}
+#endif
 
 // x <-> y swap of the 14 moments (primitive or conserved); an involution.
 __host__ __device__ constexpr int swap_xy(int m)
@@ -279,7 +292,7 @@ __device__ __forceinline__ WS5 ws5_common(double sb)
     double ss = fsqrt_pos(sb);
     w.C = fsqrt_pos(3.0 - 3.0 * sb + kTiny);
     w.E = 0.8 * w.C;
-    double B = 5.0 - 4.0 * ss + fsqrt_pos(dmax(10.0 - 16.0 * ss + 6.0 * sb, kTiny));
+    double B = 5.0 - 4.0 * ss + fsqrt_pos(floor_tiny(10.0 - 16.0 * ss + 6.0 * sb));
     double Y = B + w.E * w.E - 2.0 * w.E * fsqrt_pos(B);
     w.Y4 = 4.0 * sb * sb * Y;
     w.inv2s = 0.5 * rcp(sb);
@@ -287,7 +300,7 @@ __device__ __forceinline__ WS5 ws5_common(double sb)
 }
 __device__ __forceinline__ double ws5_lambda(const WS5& w, double sb, double qs)
 {
-    double rad = dmax(qs * qs - 0.8 * qs * sb * w.C + w.Y4, kTiny);
+    double rad = floor_tiny(qs * qs - 0.8 * qs * sb * w.C + w.Y4);
     return (qs + fsqrt_pos(rad)) * w.inv2s + w.E;
 }
 
@@ -512,7 +525,7 @@ __device__ __forceinline__ SbTerms sb_terms(double sb)
     SbTerms t;
     const double y = rsqrt_nr(sb);                     // sb >= sigma_lim > 0
     t.sb = sb; t.ss = sb * y; t.isb = y * y;
-    t.B = 5.0 - 4.0 * t.ss + fsqrt_pos(dmax(10.0 - 16.0 * t.ss + 6.0 * sb, kTiny));   // Eq 29e
+    t.B = 5.0 - 4.0 * t.ss + fsqrt_pos(floor_tiny(10.0 - 16.0 * t.ss + 6.0 * sb));   // Eq 29e
     t.sqB = fsqrt_pos(t.B);
     return t;
 }
@@ -633,7 +646,7 @@ __device__ __forceinline__ void ws14_dir(const Params& p, double Pdd, double hd,
     const double cst = 4.0 * t.sb * t.sb * (sY * sY) + p.k01 * qt2;
     const double alpha = (p.k06 * Pdd - p.k038) * Pdd + p.k035;      // Eq 29b
     const double zp = hd + alpha * qt, zm = -hd + alpha * qt;        // Eq 30: q_d -> -q_d
-    const double rp = dmax(zp * (zp - sC) + cst, kTiny), rm = dmax(zm * (zm - sC) + cst, kTiny);
+    const double rp = floor_tiny(zp * (zp - sC) + cst), rm = floor_tiny(zm * (zm - sC) + cst);
     lam_max = pref * (zp + fsqrt_pos(rp)) + E;
     lam_min_neg = pref * (zm + fsqrt_pos(rm)) + E;
 }

@@ -257,10 +257,13 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
             double WR[NV];                           // the right face state, evaluated second
             {
                 double Wm[NV], Wc[NV], Wp[NV], h[NV];
+                if (d == 0) {                        // the y stencil in x <-> y swapped numbering (L414); two copies of the
+                                                     // loads: a run-time offset costs an integer multiply-add per load
 #pragma unroll
-                for (int k = 0; k < NV; ++k) {
-                    const int o = (d == 0 ? M::cswap(k) : k) * kRW;
-                    Wm[k] = qm[o]; Wc[k] = qc[o]; Wp[k] = qp[o];
+                    for (int k = 0; k < NV; ++k) { Wm[k] = qm[M::cswap(k) * kRW]; Wc[k] = qc[M::cswap(k) * kRW]; Wp[k] = qp[M::cswap(k) * kRW]; }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) { Wm[k] = qm[k * kRW]; Wc[k] = qc[k * kRW]; Wp[k] = qp[k * kRW]; }
                 }
                 half_slopes<NV>(p, Wm, Wc, Wp, h);
                 if (d == 0) {
