@@ -127,22 +127,6 @@ __device__ __forceinline__ void tm_load(unsigned taddr, double (&v)[N])   // inc
     tm_wait_ld();
 }
 
-// split form: issue the loads early, let independent work run, then wait; the empty volatile asm after the wait
-// ties every later use of v[k] to it (nothing may read the registers before the wait)
-template <int N>
-__device__ __forceinline__ void tm_issue(unsigned taddr, double (&v)[N])
-{
-#pragma unroll
-    for (int k = 0; k < N; ++k) v[k] = tm_ld2(taddr + 2 * k);
-}
-template <int N>
-__device__ __forceinline__ void tm_arrive(double (&v)[N])
-{
-    tm_wait_ld();
-#pragma unroll
-    for (int k = 0; k < N; ++k) asm volatile("" : "+d"(v[k]));
-}
-
 // Work decomposition: item = (strip, chunk); chunk c covers rows [c ny / nchunks, (c+1) ny / nchunks).
 // EXT = false is the plain forward-Euler step with the explicit source (Ubase = nullptr,
 // dt_scale = 1, do_rate = 1, source_scheme = 0 folded at compile time); EXT = true takes them at
@@ -281,20 +265,12 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
 #pragma unroll
                     for (int k = 0; k < NV; ++k) { Wm[k] = qm[k * kRW]; Wc[k] = qc[k * kRW]; Wp[k] = qp[k * kRW]; }
                 }
-#ifdef X_EARLY
-                double hm[NV];
-                if (d == 0) tm_issue<NV>(tm + M::tm_hsv, hm);   // slope of row r-1: in flight during the slope arithmetic
-                half_slopes<NV>(p, Wm, Wc, Wp, h);
-                if (d == 0) {
-                    tm_arrive<NV>(hm);
-                    tm_store<NV>(tm + M::tm_hsv, h);
-#else
                 half_slopes<NV>(p, Wm, Wc, Wp, h);
                 if (d == 0) {
                     double hm[NV];
                     tm_load<NV>(tm + M::tm_hsv, hm);     // slope of row r-1 (garbage on the chunk's first pass: unused)
                     tm_store<NV>(tm + M::tm_hsv, h);
-#endif
+
 #pragma unroll
                     for (int k = 0; k < NV; ++k) { Wf[M::full(k)] = Wm[k] + hm[k]; WR[k] = Wc[k] - h[k]; }
                     if (r < y0) continue;            // first pass of a chunk: slope of row y0-1 only
