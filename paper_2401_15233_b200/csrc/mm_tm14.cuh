@@ -5,16 +5,20 @@
 // it shares one copy of the a(P*), b(P*) table of Eq 29c-d and one tensor-memory allocation).
 //
 // What limits this FP64 method on an SM is how many independent dependency chains are in flight: a
-// DFMA has a latency of 8 cycles and the pipe accepts one per 2 cycles and scheduler.  A face
-// evaluation (closure + flux + wave speeds, Eqs 16, 21-25, 28-31) needs ~95 registers; evaluating the
-// two faces of an interface side by side in one thread (round 1: 240 registers, 8 warps per SM) gives
-// each of 2 warps per scheduler an instruction-level parallelism of ~2.  Here every thread evaluates
-// ONE face at a time and 14-16 warps are resident.  The state that has to survive a face evaluation --
-// the finished left face of the interface (F, U, lambda: 2 NV + 2 doubles), the partial update of the
-// row (NV) and the half slopes of the previous row (NV) -- is private to a lane, and is parked in
-// TENSOR MEMORY (tcgen05.st / tcgen05.ld, 32 lanes x 128 columns per warp), Blackwell's 256 KB per SM
-// that this tensor-core-free method would otherwise leave unused: registers hold one face, shared
-// memory only what lanes exchange (the primitives ring and the rows in flight).
+// DFMA has a latency of 8 cycles and the pipe accepts one per 2 cycles and scheduler (3 when it reads
+// three distinct registers).  A face evaluation (closure + flux + wave speeds,
+// Eqs 16, 21-25, 28-31) needs ~110 registers; evaluating the two faces of an interface side by side in
+// one thread (round 1: 240 registers, 8 warps per SM) gives each of 2 warps per scheduler an
+// instruction-level parallelism of ~2.  Here every thread evaluates ONE face at a time and 16 warps of
+// 128 registers are resident (4 per scheduler; throughput scales linearly with resident warps).  The
+// state that has to survive a face evaluation -- the finished left face of the interface (F, U,
+// lambda: 2 NV + 2 doubles), the right face state (NV), the partial update of the row (NV) and the half
+// slopes of the previous row (NV) -- is private to a lane, and is parked in TENSOR MEMORY (tcgen05.st /
+// tcgen05.ld, 32 lanes x 128 columns per warp), Blackwell's 256 KB per SM that this tensor-core-free
+// method would otherwise leave unused: registers hold one face, shared memory only what lanes exchange
+// (the primitives ring and the row of own cells in flight).  The kernel sits exactly at the 128-register
+// limit: measured variants that add live values to the sweep (ghost handling, earlier tensor-memory
+// loads, part A of both faces side by side) spill and lose 3-10 %.
 //
 // The state lives in HBM twice: the conserved moments U (what the update advances, Eq 16) and the
 // primitives W = W(U) (what the reconstruction reads, L264), both written by the tail of the step that
@@ -29,6 +33,7 @@
 //                      copied by cp.async in the same group;
 // per lane, in tensor memory (columns of 32 bit, 2 per double):
 //   face  [2 NV + 2]   F_k, U_k, lambda_min, lambda_max of the left face state of the interface in work;
+//   wr    [NV]         the right face state W_C - h while the left one is evaluated;
 //   acc   [NV]         partial update of the lane's cell in the row being assembled;
 //   hsv   [NV]         half slope in y of the lane's cell in the previous row (each slope is computed once).
 // Lane L holds cell L-1 of the strip in both directions (L = 1 .. 30; lanes 0 and 31 only supply the
