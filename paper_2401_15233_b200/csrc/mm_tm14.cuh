@@ -12,7 +12,7 @@
 // instruction-level parallelism of ~2.  Here every thread evaluates ONE face at a time and 16 warps of
 // 128 registers are resident (4 per scheduler; throughput scales linearly with resident warps).  The
 // state that has to survive a face evaluation -- the finished left face of the interface (F, U,
-// lambda: 2 NV + 2 doubles), the right face state (NV), the partial update of the row (NV) and the half
+// lambda: 2 NV + 1 doubles), the right face state (NV), the partial update of the row (NV) and the half
 // slopes of the previous row (NV) -- is private to a lane, and is parked in TENSOR MEMORY (tcgen05.st /
 // tcgen05.ld, 32 lanes x 128 columns per warp), Blackwell's 256 KB per SM that this tensor-core-free
 // method would otherwise leave unused: registers hold one face, shared memory only what lanes exchange
@@ -32,7 +32,8 @@
 //   own   [NV][32]     conserved moments of the lanes' own cells in row r+1 (the base of the update),
 //                      copied by cp.async in the same group;
 // per lane, in tensor memory (columns of 32 bit, 2 per double):
-//   face  [2 NV + 2]   F_k, U_k, lambda_min, lambda_max of the left face state of the interface in work;
+//   face  [2 NV + 1]   F_k, U_k, lambda_min, lambda_max of the left face state of the interface in work
+//                      (without F_0, which is U_1: Eq 16a);
 //   wr    [NV]         the right face state W_C - h while the left one is evaluated;
 //   acc   [NV]         partial update of the lane's cell in the row being assembled;
 //   hsv   [NV]         half slope in y of the lane's cell in the previous row (each slope is computed once).
@@ -84,10 +85,10 @@ struct Mom {
     static constexpr int NW = ZS ? MM_TM_NW_ZS : MM_TM_NW_GEN;
     static constexpr size_t smem_bytes = ((size_t)AbTable::kDoubles + (size_t)NW * warp_smem_doubles) * sizeof(double) + 16;
     // tensor-memory columns of a lane: [face | acc | hsv]
-    static constexpr int tm_face = 0, tm_acc = 2 * (2 * NV + 2), tm_hsv = tm_acc + 2 * NV, tm_wr = tm_hsv + 2 * NV,
+    static constexpr int tm_face = 0, tm_acc = 2 * (2 * NV + 1), tm_hsv = tm_acc + 2 * NV, tm_wr = tm_hsv + 2 * NV,
                          tm_cols = tm_wr + 2 * NV;
     // a warp may only touch the 32-lane quarter warp % 4: the (NW + 3) / 4 warps of a quarter split its 512 columns
-    static constexpr int tm_stride = (512 / ((NW + 3) / 4)) & ~7;
+    static constexpr int tm_stride = (512 / ((NW + 3) / 4)) & ~1;
     static_assert(tm_cols <= tm_stride, "tensor-memory columns of a warp");
 };
 
@@ -151,7 +152,7 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
     const int do_rate = EXT ? do_rate_ : 1;
     using Z = typename std::conditional<ZS, zero_t, double>::type;
     using M = Mom<ZS>;
-    constexpr int NM = 14, NV = M::NV, NF = 2 * NV + 2, RS = NV * kRW;   // RS: doubles per staged row
+    constexpr int NM = 14, NV = M::NV, NF = 2 * NV + 1, RS = NV * kRW;   // RS: doubles per staged row
     extern __shared__ __align__(16) double smem[];
     // the warp index through a shuffle: the compiler then knows it is warp-uniform and keeps what derives
     // from it (buffer bases, tensor-memory addresses) in uniform registers
@@ -296,10 +297,11 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
             for (int side = 0; side < 2; ++side) {
                 eval_face14<Z>(p, Wf, F, U, lmin, lmax);
                 if (side == 0) {
-                    double park[NF];
+                    double park[NF];                 // [U_0 | F_k, U_k (k >= 1) | lambda_min, lambda_max]: F_0 = U_1 (Eq 16a) is not parked
+                    park[0] = U[0];
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) { park[2 * k] = F[M::full(k)]; park[2 * k + 1] = U[M::full(k)]; }
-                    park[2 * NV] = lmin; park[2 * NV + 1] = lmax;
+                    for (int k = 1; k < NV; ++k) { park[2 * k - 1] = F[M::full(k)]; park[2 * k] = U[M::full(k)]; }
+                    park[2 * NV - 1] = lmin; park[2 * NV] = lmax;
                     tm_store<NF>(tm + M::tm_face, park);
                     double wr[NV];
                     tm_wait_st();
@@ -313,13 +315,16 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
                 double L[NF];
                 tm_wait_st();
                 tm_load<NF>(tm + M::tm_face, L);
-                const double lminL = L[2 * NV], lmaxL = L[2 * NV + 1];
+                const double lminL = L[2 * NV - 1], lmaxL = L[2 * NV];
+                // left face: U_k = LU(k), F_k = LF(k) with F_0 = U_1
+#define MM_LU(k) L[(k) == 0 ? 0 : 2 * (k)]
+#define MM_LF(k) L[(k) == 0 ? 2 : 2 * (k) - 1]
                 if (p.flux == 1) {
                     const double S = dmax(dmax(fabs(lminL), fabs(lmaxL)), dmax(fabs(lmin), fabs(lmax)));
 #pragma unroll
                     for (int k = 0; k < NV; ++k) {
                         const int m = M::full(k);
-                        Fh[k] = 0.5 * (L[2 * k] + F[m]) - 0.5 * S * (U[m] - L[2 * k + 1]);
+                        Fh[k] = 0.5 * (MM_LF(k) + F[m]) - 0.5 * S * (U[m] - MM_LU(k));
                     }
                 } else {
                     const double SL = dmin(dmin(lminL, lmin), 0.0), SR = dmax(dmax(lmaxL, lmax), 0.0);
@@ -327,9 +332,11 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
 #pragma unroll
                     for (int k = 0; k < NV; ++k) {
                         const int m = M::full(k);
-                        Fh[k] = hll1(cL, cR, cU, L[2 * k], F[m], L[2 * k + 1], U[m]);
+                        Fh[k] = hll1(cL, cR, cU, MM_LF(k), F[m], MM_LU(k), U[m]);
                     }
                 }
+#undef MM_LU
+#undef MM_LF
             }
             if (d == 0) {
                 double G[NV];                        // back to unswapped numbering (L414)
