@@ -101,8 +101,10 @@ typedef struct {
     void *stream;         /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
 } mm_options;
 
-/* Bytes of device workspace mm_create needs for this grid (two padded state copies, boundary
- * tables, control block, wave-speed table, dt history).  0 on invalid grid. */
+/* Bytes of device workspace mm_create needs for this grid: two padded state copies (the 14-moment
+ * system keeps each copy as conserved moments U and as primitives W(U), 4 x 14 planes in all; the
+ * 5-moment system 2 x 5 planes), boundary tables, control block, wave-speed table, dt history.
+ * 0 on invalid grid. */
 size_t mm_workspace_bytes(const mm_grid *grid);
 
 /* Build a solver on caller-provided device memory (problem statement of section 3 L250 and section 6
@@ -113,7 +115,9 @@ int mm_create(mm_solver **out, const mm_grid *grid, const mm_gas *gas, const mm_
 
 /* Load the interior state (conserved resp. primitive moments, [nmom][ny][nx]), fill the ghost
  * cells and run the CFL reduction; resets t = 0, steps = 0.  Host buffers are copied with
- * cudaMemcpyAsync on the solver's stream (pin them for true overlap). */
+ * cudaMemcpyAsync on the solver's stream (pin them for true overlap).  The conserved moments given
+ * to mm_set_state are stored as they are (mm_get_state returns the same bits); mm_get_state +
+ * mm_get_info followed by mm_set_state + mm_set_clock on a new solver resumes a run bit for bit. */
 int mm_set_state(mm_solver *s, const double *U, int on_device);
 int mm_set_state_prim(mm_solver *s, const double *W, int on_device);
 
