@@ -57,11 +57,12 @@ def inflow_scout_dt(mmo, prob, n, nsteps, cfl):
 
 
 # --------------------------------------------------------------- the bar at the headline size
-def test_C4_full_grid_2048_100_steps(mm, mmo):
-    """configs[3] as bench.py runs it (seeded +-1 % density, Kn 0.1, z-symmetric kernel variant, bench
+@pytest.mark.parametrize("Kn", [0.1, 1.0])
+def test_C4_full_grid_2048_100_steps(mm, mmo, Kn):
+    """configs[3] as bench.py runs it (seeded +-1 % density, Kn 0.1 and 1, z-symmetric kernel variant, bench
     launch decomposition): 100 fixed-dt steps, every one of the 4 194 304 cells, all 14 moments."""
     n, nsteps = 2048, 100
-    prob = wl.crossed_jets(n, Kn=0.1, perturb=0.01)
+    prob = wl.crossed_jets(n, Kn=Kn, perturb=0.01)
     so = oracle_solver(mmo, prob)
     sg = mm.Solver.from_problem(prob)
     assert sg.fast_path_active
