@@ -19,7 +19,9 @@
  *     mm_bc are copied at mm_create.
  *   - the library never allocates device memory: the caller hands in `d_workspace`
  *     (>= mm_workspace_bytes(), 256-byte aligned, e.g. a torch uint8 tensor) and a stream;
- *     all work is enqueued on that stream, nothing synchronises unless stated.
+ *     all work is enqueued on that stream, nothing synchronises unless stated.  A caller that has
+ *     no way of obtaining a workspace uses mm_static5_run (end of this header), whose scratch is a
+ *     fixed array inside the library image.
  *   - solver objects are independent; one object is not thread-safe.
  *
  * Moment order (structure of arrays, fp64), field arrays are [moment][ny][nx], interior cells:
@@ -40,7 +42,7 @@ extern "C" {
 #endif
 
 typedef enum { MM_OK = 0, MM_EINVAL = -1, MM_EWORKSPACE = -2, MM_ECUDA = -3,
-               MM_ENONFINITE = -4 } mm_status;
+               MM_ENONFINITE = -4, MM_ETOOLARGE = -5 /* mm_static5_run only */ } mm_status;
 
 enum { MM_SYS5_1D = 5, MM_SYS14_2D = 14 };                       /* section 2.3 / 2.4 */
 enum { MM_TAU_NONE = 0, MM_TAU_CONST = 1, MM_TAU_KN = 2 };
@@ -203,6 +205,52 @@ void mm_batch5_destroy(mm_batch5 *b);
 
 void mm_destroy(mm_solver *s);
 const char *mm_strerror(int status);
+
+/* ---- mm_static5_run: a whole 1-D 5-moment run for callers that cannot provide a workspace.
+ *
+ * Everything above needs `d_workspace`, i.e. a caller able to obtain device memory of a size the library
+ * dictates.  Some users of this library are not: a routine called back from inside somebody else's
+ * solver or coupling framework is handed the device (or host) arrays of its input and output and
+ * nothing else -- the host application owns the device-memory pool, has often reserved all of the
+ * GPU for it, and a raw runtime allocation from the callee then fails or is forbidden by the host's
+ * rules; a caller sitting in a time-critical loop cannot afford the device-wide synchronisation a
+ * runtime allocation or release implies; and a C or Fortran driver that links this library alone has
+ * no CUDA runtime of its own to allocate with.  For them the scratch of the 5-moment step (control
+ * block, boundary table, dt history and the two padded copies of the state that k_step5 ping-pongs
+ * between) lives in ONE file-scope device array of MM_STATIC5_SCRATCH_BYTES (4 MiB) compiled into
+ * libmm.so.  Every GPU whose context loads the library carries these 4 MiB until the process exits,
+ * whether or not this function is ever called; that is the price, and the reason the limit is modest:
+ *   nx <= MM_STATIC5_MAX_NX (8192 cells); larger nx returns MM_ETOOLARGE before any CUDA call.
+ *
+ * What it does: the same launches as mm_create(MM_SYS5_1D) + mm_set_state_prim(W0) + n steps
+ * (dt > 0: n steps of that fixed dt, mm_step_fixed_dt; otherwise n CFL steps at Courant number cfl,
+ * mm_step) + mm_get_state(U), on options->stream, with the built-in array as the workspace.  The
+ * results are those of that sequence, bit for bit.
+ *   W0      primitives (rho, u, P, q, r), [5][nx]          U   conserved moments out, [5][nx]
+ *   on_device  1: W0 and U are device pointers, 0: host pointers (copied on the stream; no staging
+ *           buffer is allocated, the idle state copy inside the array serves)
+ *   bcs     two sides (xlo, xhi) as in mm_create, or NULL for transmissive ends (L426)
+ *   t_end   host pointer, receives the time reached; may be NULL
+ * Returns MM_OK, MM_EINVAL, MM_ETOOLARGE, MM_ECUDA (also: no device -- there is no CPU path) or
+ * MM_ENONFINITE as mm_get_info does.  Synchronises the stream before returning.  It performs no device
+ * or pinned-host allocation and releases none; host-side it builds and frees one small solver object.
+ *
+ * Sharing.  There is one array per device and process, and every call on that device uses it.  It keeps
+ * whatever the previous call left: each call therefore zero-fills the part it is about to use (control
+ * block, accumulators, tables, both state copies) on the stream before anything reads it.  Two calls
+ * whose GPU work overlaps would overwrite each other's state -- a race with silently wrong numbers.  The
+ * function prevents that inside one process by holding a lock from its first launch until its stream has
+ * drained; nothing can be done about it from here if the array were reached by other means, so do not.
+ *
+ * First call on a device.  The device address of the array is looked up (and the module holding it is
+ * loaded) the first time the function runs with that device current; later calls on that device reuse
+ * it.  Make that first call during start-up, outside any stream capture: loading a module is not a
+ * stream operation. */
+#define MM_STATIC5_MAX_NX 8192
+#define MM_STATIC5_SCRATCH_BYTES (4u << 20)
+int mm_static5_run(int nx, double x0, double x1, const mm_collision *collision, const mm_bc *bcs,
+                   const mm_options *options, const double *W0, int n, double cfl, double dt,
+                   double *U, int on_device, double *t_end);
 
 #ifdef __cplusplus
 }

@@ -7,6 +7,7 @@
 
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -766,8 +767,79 @@ const char* mm_strerror(int status)
     case MM_EWORKSPACE: return "workspace missing, too small or not 256-byte aligned";
     case MM_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
     case MM_ENONFINITE: return "CFL reduction met rho <= 0, P <= 0 or a non-finite wave speed";
+    case MM_ETOOLARGE: return "problem larger than the library's built-in scratch: mm_static5_run takes at most "
+                              "MM_STATIC5_MAX_NX = 8192 cells (use mm_create with a workspace of your own beyond that)";
     default: return "unknown status";
     }
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------- run without a caller workspace
+// mm_static5_run (include/mm.h) serves callers that can hand over their input and output arrays but no
+// device workspace: callbacks living inside a host application that owns all device memory, loops that
+// must not hit the device-wide synchronisation of a runtime allocation, drivers without a CUDA runtime of
+// their own.  The scratch of the 5-moment step -- everything mm_workspace_bytes() would have asked the
+// caller for -- is this one array in the library image instead: 4 MiB on every GPU that loads libmm.so,
+// until the process exits.
+namespace {
+
+static __device__ __align__(256) unsigned char g_static5_scratch[MM_STATIC5_SCRATCH_BYTES];
+
+// In host code `g_static5_scratch` is only the handle the runtime knows the array by, not an address a
+// kernel could use.  The usable device address differs per device; it is looked up once per device, with
+// that device current, and kept here.
+constexpr int kStatic5MaxDevices = 64;
+void* g_static5_addr[kStatic5MaxDevices];
+std::mutex g_static5_mu;        // one call at a time: all calls on a device share the array
+
+int static5_scratch_address(void** out)
+{
+    int dev = -1;
+    MM_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStatic5MaxDevices) return MM_EINVAL;
+    if (!g_static5_addr[dev]) {
+        void* p = nullptr;
+        MM_CUDA(cudaGetSymbolAddress(&p, g_static5_scratch));
+        if (!p) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_static5_scratch)");
+        g_static5_addr[dev] = p;
+    }
+    *out = g_static5_addr[dev];
+    return MM_OK;
+}
+
+}  // namespace
+
+extern "C" int mm_static5_run(int nx, double x0, double x1, const mm_collision* collision, const mm_bc* bcs,
+                              const mm_options* options, const double* W0, int n, double cfl, double dt,
+                              double* U, int on_device, double* t_end)
+{
+    if (!collision || !options || !W0 || !U || nx < 1 || n < 0) return MM_EINVAL;
+    if (!(dt > 0.0) && !(cfl > 0.0)) return MM_EINVAL;
+    if (nx > MM_STATIC5_MAX_NX) return MM_ETOOLARGE;            // before any CUDA call
+    const mm_grid g = {MM_SYS5_1D, nx, 1, x0, x1, 0.0, 1.0};
+    Layout L;
+    if (!make_layout(&g, &L)) return MM_EINVAL;
+    if (L.total > (size_t)MM_STATIC5_SCRATCH_BYTES) return MM_ETOOLARGE;
+    mm_bc sides[4];
+    memset(sides, 0, sizeof sides);                              // MM_BC_TRANSMISSIVE
+    if (bcs) { sides[0] = bcs[0]; sides[1] = bcs[1]; }
+
+    std::lock_guard<std::mutex> lock(g_static5_mu);
+    void* scratch = nullptr;
+    int rc = static5_scratch_address(&scratch);                  // first call on this device: module load + lookup
+    if (rc) return rc;
+    // mm_create zero-fills the L.total bytes this problem uses (the array still holds the previous call's
+    // control block, tables and states) and rebuilds the boundary table; the solver object is host memory.
+    mm_solver* s = nullptr;
+    if ((rc = mm_create(&s, &g, nullptr, collision, sides, options, scratch, MM_STATIC5_SCRATCH_BYTES))) return rc;
+    rc = mm_set_state_prim(s, W0, on_device);
+    if (!rc) rc = dt > 0.0 ? mm_step_fixed_dt(s, n, dt) : mm_step(s, n, cfl);
+    if (!rc) rc = mm_get_state(s, U, on_device);
+    if (!rc) rc = mm_get_info(s, t_end, nullptr, nullptr, nullptr);
+    // whatever happened, nothing of this call may still be running on the array when the lock is released
+    const cudaError_t e = cudaStreamSynchronize(s->stream);
+    mm_destroy(s);
+    if (!rc && e != cudaSuccess) rc = cuda_fail(e, "mm_static5_run: cudaStreamSynchronize");
+    return rc;
+}

@@ -21,8 +21,9 @@ LIM_NONE, LIM_MINMOD, LIM_VANALBADA = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
 SRC_EXPLICIT, SRC_POINT_IMPLICIT = 0, 1      # BGK source: forward Euler | point-implicit
 TIME_EULER, TIME_MIDPOINT = 0, 1             # forward Euler | midpoint (2nd-order RK)
-OK, EINVAL, EWORKSPACE, ECUDA, ENONFINITE = 0, -1, -2, -3, -4
+OK, EINVAL, EWORKSPACE, ECUDA, ENONFINITE, ETOOLARGE = 0, -1, -2, -3, -4, -5
 MAX_BANDS = 8
+STATIC5_MAX_NX = 8192                         # mm_static5_run: cells the built-in 4 MiB scratch holds
 
 EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim", "mm_step",
            "mm_step_fixed_dt", "mm_advance_to", "mm_get_state", "mm_get_state_prim", "mm_get_info",
@@ -31,7 +32,7 @@ EXPORTS = ["mm_workspace_bytes", "mm_create", "mm_set_state", "mm_set_state_prim
            "mm_destroy", "mm_strerror",
            "mm_batch5_workspace_bytes", "mm_batch5_create", "mm_batch5_set_state_prim", "mm_batch5_step",
            "mm_batch5_step_fixed_dt", "mm_batch5_advance_to", "mm_batch5_get_state", "mm_batch5_get_info",
-           "mm_batch5_launch_count", "mm_batch5_destroy"]
+           "mm_batch5_launch_count", "mm_batch5_destroy", "mm_static5_run"]
 BENCH_EXPORTS = ["mm_measure_fp64_peak", "mm_measure_fp64_operand_rates", "mm_selftest_fastmath"]          # include/mm_bench.h, libmm_bench.so
 
 _dp = C.POINTER(C.c_double)
@@ -116,6 +117,9 @@ def lib() -> C.CDLL:
     L.mm_batch5_launch_count.restype, L.mm_batch5_launch_count.argtypes = C.c_longlong, [vp]
     L.mm_batch5_destroy.restype, L.mm_batch5_destroy.argtypes = None, [vp]
     L.mm_strerror.restype, L.mm_strerror.argtypes = C.c_char_p, [i]
+    L.mm_static5_run.restype = i
+    L.mm_static5_run.argtypes = [i, d, d, C.POINTER(mm_collision), C.POINTER(mm_bc), C.POINTER(mm_options),
+                                 vp, i, d, d, vp, i, _dp]
     _lib = L
     return L
 
@@ -188,6 +192,55 @@ def mm_selftest_fastmath(n: int = 1 << 22, stream=None):
     out = (C.c_double * 3)()
     _check(bench_lib().mm_selftest_fastmath(C.c_void_p(st.cuda_stream), n, out))
     return tuple(out)
+
+
+def static5_run(W0, n: int, cfl: float = 0.0, dt: float = 0.0, extent=(0.0, 1.0), collision: Optional[dict] = None,
+                sigma_lim: float = 1e-4, ws_scale: float = 1.0, limiter: int = LIM_MINMOD, shared_limiter: int = 0,
+                flux: int = FLUX_HLL, source_scheme: int = SRC_EXPLICIT, time_scheme: int = TIME_EULER,
+                periodic: bool = False, out=None, stream=None):
+    """mm_static5_run (include/mm.h): n steps of a 1-D 5-moment tube of nx <= STATIC5_MAX_NX cells with no
+    workspace from the caller -- the scratch is a 4 MiB array built into libmm.so, shared by every call on
+    the device.  For callers that hold only their input and output arrays and cannot get device memory of
+    their own (see the header for who they are).  W0: primitives [5][nx], numpy array (host path) or CUDA
+    float64 tensor (device path); returns (U, t) with U of the same kind, conserved moments [5][nx].
+    dt > 0: fixed time step; otherwise CFL steps at Courant number cfl.  Ends are transmissive, or
+    periodic.  This wrapper allocates only `out` when none is given; pass `out` to allocate nothing."""
+    import torch
+    if not torch.cuda.is_available():
+        raise MMError(ECUDA, "no CUDA device: the moment-method library has no CPU path")
+    on_device = isinstance(W0, torch.Tensor) and W0.is_cuda
+    if on_device:
+        if W0.dtype != torch.float64 or not W0.is_contiguous() or W0.numel() % 5:
+            raise ValueError("W0 must be a contiguous float64 tensor [5, nx]")
+        nx = W0.numel() // 5
+        if out is None:
+            out = torch.empty((5, nx), dtype=torch.float64, device=W0.device)
+        elif not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64
+                  and out.is_contiguous() and out.numel() == 5 * nx):
+            raise ValueError("out must be a contiguous CUDA float64 tensor [5, nx]")
+        src, dst = C.c_void_p(W0.data_ptr()), C.c_void_p(out.data_ptr())
+    else:
+        W0 = _darr(W0)
+        if W0.size % 5:
+            raise ValueError("W0 must be [5, nx]")
+        nx = W0.size // 5
+        if out is None:
+            out = np.empty((5, nx))
+        elif out.dtype != np.float64 or not out.flags.c_contiguous or out.size != 5 * nx:
+            raise ValueError("out must be a contiguous float64 array [5, nx]")
+        src, dst = C.c_void_p(W0.ctypes.data), C.c_void_p(out.ctypes.data)
+    col = collision or {"model": TAU_NONE}
+    c = mm_collision(col.get("model", TAU_NONE), col.get("tau", 0.0), col.get("Kn", 0.0),
+                     col.get("L_ref", 1.0), col.get("rho_ref", 1.0))
+    sides = (mm_bc * 2)()
+    sides[0].type = sides[1].type = BC_PERIODIC if periodic else BC_TRANSMISSIVE
+    st = stream if stream is not None else torch.cuda.current_stream()
+    o = mm_options(sigma_lim, ws_scale, limiter, shared_limiter, flux, source_scheme, time_scheme,
+                   C.c_void_p(st.cuda_stream))
+    t = C.c_double()
+    _check(lib().mm_static5_run(nx, extent[0], extent[1], C.byref(c), sides, C.byref(o), src, n, cfl, dt,
+                                dst, int(on_device), C.byref(t)))
+    return out, t.value
 
 
 class Solver:
