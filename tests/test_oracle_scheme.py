@@ -513,3 +513,50 @@ def test_face_states_shared_limiter_is_what_the_step_uses(mmo):
                               mmo.prim2cons(WL), mmo.prim2cons(WR), a[0], a[1], b[0], b[1])
     expect = U0 - dt * nx * (np.roll(F, -1, axis=1) - F)
     np.testing.assert_allclose(U1, expect, rtol=1e-13, atol=1e-15)
+
+
+# ------------------------------------------------- 2-D CFL rate (section 6.1, Fig 14; reading R13)
+LAMBDA_EQ = 2.18259874765634      # Eq 29 at equilibrium, sigma_bar = 1e-4 (mpmath; SURVEY.md section 8(c), row "wave speeds")
+
+
+@pytest.mark.parametrize("u, winner", [((0.3, 0.1), "y"), ((6.0, 0.1), "x"), ((-6.0, 0.1), "x"), ((0.3, -2.0), "y")])
+def test_cfl_dt_2d_anisotropic_cells(mmo, u, winner):
+    """dt = cfl / max over cells of max(s_x/dx, s_y/dy) with s_d = |u_d| + lambda* c for a uniform Maxwellian
+    (q = 0: the two speeds of Eq 29 are u_d +- lambda* c), on cells with dx = 2 dy: a scheme that divides both
+    directions by dx, takes the minimum, or forgets a direction gives another number in one of the cases."""
+    rho, T = 0.7, 1.3
+    c = math.sqrt(T)
+    nx, ny = 8, 6
+    W = wl.maxwellian(wl.SYS14, np.full((ny, nx), rho), (u[0], u[1], 0.0), T)
+    dx, dy = 2.0 / nx, 0.75 / ny
+    assert dx == 2.0 * dy
+    s = mmo.Solver(14, nx, ny, extent=(0.0, 2.0, 0.0, 0.75), collision=dict(model=wl.TAU_NONE),
+                   bcs=[dict(type=wl.BC_PERIODIC)] * 4, sigma_lim=1e-4)
+    s.set_state_prim(W)
+    rx, ry = (abs(u[0]) + LAMBDA_EQ * c) / dx, (abs(u[1]) + LAMBDA_EQ * c) / dy
+    assert (rx > ry) == (winner == "x") and abs(rx - ry) > 0.1 * max(rx, ry)
+    for cfl in (0.5, 0.4):
+        assert s.cfl_dt(cfl) == pytest.approx(cfl / max(rx, ry), rel=1e-12)
+    # the step taken by step(1, cfl) is that dt (L434: "imposing a Courant number of 0.5")
+    s.step(1, 0.5)
+    assert s.info()["last_dt"] == pytest.approx(0.5 / max(rx, ry), rel=1e-12)
+
+
+def test_cfl_dt_is_set_by_a_dirichlet_ghost_state(mmo):
+    """Reading R13: ghost cells take part in the CFL maximum.  Gas at rest (rho = T = 1) on 20 x 20 unit-square cells,
+    dx = dy = 0.05; one Dirichlet band on the left side holds a Maxwellian moving at u_x = 5.  Interior cells alone
+    would give dt = 0.4 * 0.05 / 2.18259874765634 = 9.1634e-3; with the ghost state the fastest cell has
+    s_x = 5 + 2.18259874765634, so dt = 0.4 * 0.05 / 7.18259874765634 = 2.7845075e-3."""
+    n = 20
+    rest = wl.maxwellian(wl.SYS14, 1.0, (0.0, 0.0, 0.0), 1.0)
+    fast = wl.maxwellian(wl.SYS14, 1.0, (5.0, 0.0, 0.0), 1.0)
+    bcs = [dict(type=wl.BC_DIRICHLET, bands=[(0.3, 0.4, fast)], default=rest),
+           dict(type=wl.BC_TRANSMISSIVE), dict(type=wl.BC_TRANSMISSIVE), dict(type=wl.BC_TRANSMISSIVE)]
+    s = mmo.Solver(14, n, n, extent=(0.0, 1.0, 0.0, 1.0), collision=dict(model=wl.TAU_NONE), bcs=bcs, sigma_lim=1e-4)
+    s.set_state_prim(wl.maxwellian(wl.SYS14, np.ones((n, n)), (0.0, 0.0, 0.0), 1.0))
+    assert s.cfl_dt(0.4) == pytest.approx(2.784507488536227e-3, rel=1e-12)
+    # without a band in reach of any cell centre the interior value is back
+    bcs[0] = dict(type=wl.BC_DIRICHLET, bands=[(0.33, 0.37, fast)], default=rest)     # cell centres 0.325, 0.375: none inside
+    s2 = mmo.Solver(14, n, n, extent=(0.0, 1.0, 0.0, 1.0), collision=dict(model=wl.TAU_NONE), bcs=bcs, sigma_lim=1e-4)
+    s2.set_state_prim(wl.maxwellian(wl.SYS14, np.ones((n, n)), (0.0, 0.0, 0.0), 1.0))
+    assert s2.cfl_dt(0.4) == pytest.approx(9.163388378865272e-3, rel=1e-12)
