@@ -279,7 +279,10 @@ k_step14_tm(const Params pg, const double* __restrict__ Win, const double* __res
 
 #pragma unroll
                     for (int k = 0; k < NV; ++k) { Wf[M::full(k)] = Wm[k] + hm[k]; WR[k] = Wc[k] - h[k]; }
-                    if (r < y0) continue;            // first pass of a chunk: slope of row y0-1 only
+                    if (r < y0) {                    // first pass of a chunk: slope of row y0-1 only.  The next pass loads it
+                        tm_wait_st();                // back before any other wait::st: tcgen05.st -> tcgen05.ld of one thread
+                        continue;                    // is not ordered without it
+                    }
                     tm_store<NV>(tm + M::tm_wr, WR);
                 } else {
 #pragma unroll
