@@ -177,6 +177,31 @@ def random_smooth14(nx: int, ny: int, seed: int = SEED, amp: float = 0.2, period
     return _problem(SYS14, nx, ny, (0.0, 1.0, 0.0, ny / nx), col, bcs, W0, **options)
 
 
+def anisotropic14(nx: int, ny: int, axis: int = 0, ratio: float = 0.025, seed: int = SEED, amp: float = 0.1,
+                  zsym: bool = False, Kn=None, **options):
+    """Smooth periodic state whose pressure tensor is strongly anisotropic: the normal pressure along `axis`
+    (0: P_xx, 1: P_yy) is `ratio` x the hydrostatic pressure, the other two share the rest, so that
+    P_dd* = P_dd / P < 1/32 everywhere along that direction -- below the range a tabulated a(P*), b(P*) of
+    Eq 29c-d would normally cover.  R_iijj is 1.3 x the fourth moment of the Gaussian with this pressure tensor,
+    ((tr P)^2 + 2 P_ij P_ij) / rho, which keeps the state inside the realizability bound of Eq 19; everything
+    else as random_smooth14."""
+    prob = random_smooth14(nx, ny, seed=seed, amp=amp, zsym=zsym, Kn=Kn, **options)
+    W0 = prob["W0"]
+    rho = W0[0]
+    Ph = (W0[4] + W0[7] + W0[9]) / 3.0
+    diag = (4, 7, 9)
+    small = diag[axis]
+    shape = W0[small] / Ph                              # 1 + a few percent, smooth
+    for m in diag:
+        W0[m] = Ph * (ratio * shape if m == small else 0.5 * (3.0 - ratio * shape))
+    W0[5] *= 0.2; W0[6] *= 0.2; W0[8] *= 0.2            # keep P positive definite next to the small eigenvalue
+    W0[10] *= 0.3; W0[11] *= 0.3; W0[12] *= 0.3
+    trP = W0[4] + W0[7] + W0[9]
+    PP = W0[4] ** 2 + W0[7] ** 2 + W0[9] ** 2 + 2.0 * (W0[5] ** 2 + W0[6] ** 2 + W0[8] ** 2)
+    W0[13] = 1.3 * (trP * trP + 2.0 * PP) / rho
+    return prob
+
+
 def random_smooth5(nx: int, seed: int = SEED, amp: float = 0.2, periodic: bool = True, Kn=None,
                    **options):
     """Smooth non-equilibrium 5-moment state on a periodic interval."""

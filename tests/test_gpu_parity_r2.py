@@ -191,6 +191,48 @@ def test_resync_sod14_collisionless_front(mm, mmo):
     resync_steps(mm, mmo, prob, U0, 30, dt, fast=True)
 
 
+@pytest.mark.parametrize("limiter", [wl.LIM_MINMOD, wl.LIM_VANALBADA])
+def test_resync_smooth14_general_variant_shared_limiter(mm, mmo, limiter):
+    """The one combination that only had a condition-aware bar: fully 3-D data (non-zero u_z, P_xz, P_yz, q_z),
+    the general kernel variant and ONE limiter value for all 14 primitives ("the most stringent").
+    30 re-synchronised steps of random_smooth14(70, 37) at the flat 1e-10."""
+    prob = wl.random_smooth14(70, 37, Kn=0.1, limiter=limiter, shared_limiter=1)
+    assert all(np.abs(prob["W0"][m]).max() > 1e-3 for m in (3, 6, 8, 12))
+    so = oracle_solver(mmo, prob)
+    U0 = so.get_state()
+    dt = 0.5 * so.cfl_dt(0.4)
+    sg = mm.Solver.from_problem(prob)
+    assert not sg.fast_path_active                          # z-odd moments present: the general variant runs
+    resync_steps(mm, mmo, prob, U0, 30, dt)
+
+
+@pytest.mark.parametrize("axis, zsym", [(0, True), (1, True), (0, False), (1, False)])
+def test_anisotropic_pressure_takes_the_direct_wave_speed_path(mm, mmo, axis, zsym):
+    """P_dd* < 1/32 along one direction: every face evaluation of that direction inside the step kernel leaves
+    the a(P*), b(P*) table (Eq 29c-d) and redoes its wave speeds with the formulas themselves, lane by lane,
+    right before the warp-collective tensor-memory instructions.  25 steps at fixed dt, both kernel variants."""
+    prob = wl.anisotropic14(70, 37, axis=axis, zsym=zsym, ratio=0.02)      # collisionless: the anisotropy persists
+    W0 = prob["W0"]
+    Ph = (W0[4] + W0[7] + W0[9]) / 3.0
+    assert (W0[(4, 7)[axis]] / Ph).max() < 1.0 / 32.0
+    so = oracle_solver(mmo, prob)
+    dts = []
+    for _ in range(25):
+        so.step(1, 0.4)
+        dts.append(so.info()["last_dt"])
+    Wend = so.get_state_prim()
+    assert (Wend[(4, 7)[axis]] / ((Wend[4] + Wend[7] + Wend[9]) / 3.0)).max() < 1.0 / 32.0    # every cell still out of the table's range
+    dt = 0.5 * min(dts)
+    so = oracle_solver(mmo, prob)
+    sg = mm.Solver.from_problem(prob)
+    assert sg.fast_path_active == zsym
+    so.step_fixed_dt(25, dt); sg.step_fixed_dt(25, dt)
+    Uo, Ug = so.get_state(), sg.get_state()
+    assert np.all(np.isfinite(Uo))
+    e = moment_errors(Ug, Uo)
+    assert e.max() <= TOL, e
+
+
 # ------------------------------------------------------------------------------ boundary
 def test_maxwellian_dirichlet_states_use_R_gas(mm, mmo):
     """mm_gas (include/mm.h): Dirichlet states given as (rho, u, T) are expanded on the device to the
