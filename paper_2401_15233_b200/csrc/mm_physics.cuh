@@ -136,8 +136,12 @@ static const double kTiny = 0x1p-996;
 constexpr double kTiny = 0x1p-996;
 #endif
 // max(x, kTiny) for the floored radicands (R6), decided on the high word with integer instructions: for x >= kTiny
-// (and for NaN, which passes through) the signed high word is >= that of kTiny; negative, zero and subnormal x have
-// a smaller one.  Same values as dmax(x, kTiny), without an FP64-pipe compare.
+// the signed high word is >= that of kTiny; negative, zero and subnormal x have a smaller one.  A NaN passes through
+// only with its sign bit clear; the canonical NaN of CUDA arithmetic (0xFFF8000000000000, sign bit set) has a negative
+// high word and comes out as kTiny -- exactly what dmax(x, kTiny) = (x > kTiny ? x : kTiny) returns for a NaN too, so
+// the values are those of dmax without an FP64-pipe compare.  A failed state is therefore not detected through a
+// floored radicand: the CFL reduction flags it through rho <= 0, P <= 0 or a non-finite speed from the other terms
+// (C, E and the prefactor of Eq 29 carry the NaN).
 #ifdef MM_OPCOUNT_HOST
 __forceinline__ double floor_tiny(double x) { return dmax(x, kTiny); }
 #else
@@ -817,6 +821,9 @@ __device__ __forceinline__ void eval_face14(const Params& p, const double (&W)[1
     eval_face14_A<Z, true>(p, W, a, lmin, lmax);
     eval_face14_B<Z>(p, W, a, F, U);
     if (!ab_in_table(a.s.pxx)) face14_speeds_direct<Z>(p, W, a, lmin, lmax);
+    // the fallback diverges per lane (and calls a function); the step kernel's warp-collective tensor-memory
+    // instructions that follow need all 32 lanes back together
+    __syncwarp();
 #else
     eval_face14_A<Z>(p, W, a, lmin, lmax);
     eval_face14_B<Z>(p, W, a, F, U);
