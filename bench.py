@@ -35,7 +35,7 @@ UNIT = "cell-updates/s"
 CFL = 0.4
 
 
-def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14):
+def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14, limiter: int = 1, flux: int = 0):
     """Algorithmic FP64 operations per cell update (each + - * / sqrt exp
     pow = 1, so a(P*), b(P*) of Eq 29c-d are 10 per call whatever the kernel's table evaluation executes).
     -> (count of the formulation the CUDA path runs, the same with the table evaluation as executed,
@@ -44,8 +44,10 @@ def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14):
     only because of an implementation choice, are not credited to it.  All are produced by committed
     counting builds, not typed in."""
     from paper_2401_15233_b200 import build_ext
+    # counted for the limiter and the flux function that ran (van Albada / Rusanov carry a key suffix, opcount.txt)
     key = (f"kernel_flops_per_cell_update_{system}_" + ("zsym_" if zsym and system == 14 else "")
-           + ("shared_limiter" if shared_limiter else "per_variable_limiter"))
+           + ("shared_limiter" if shared_limiter else "per_variable_limiter")
+           + ("_vanalbada" if limiter == wl.LIM_VANALBADA else "") + ("_rusanov" if flux == wl.FLUX_RUSANOV else ""))
     oc = build_ext.read_opcount()
     k = oc[key]
     o = None
@@ -321,7 +323,9 @@ def run_gpu(args):
     finite = bool(torch.isfinite(U_host).all())
 
     if rank == 0:
-        fpc, fpc_exec, fpc_oracle = flops_per_cell_update(bool(prob["options"]["shared_limiter"]), s.fast_path_active, nm)
+        opt = prob["options"]
+        fpc, fpc_exec, fpc_oracle = flops_per_cell_update(bool(opt["shared_limiter"]), s.fast_path_active, nm,
+                                                          limiter=opt["limiter"], flux=opt["flux"])
         # the probe also reports the SM clock it ran at (cycle counter / global timer inside the kernel)
         peak_tf, peak_mhz = mm.mm_measure_fp64_peak(5, with_clock=True)
         # the pipe's instruction rates when the register-reuse cache cannot supply operands
@@ -332,6 +336,11 @@ def run_gpu(args):
         achieved_tf = fpc * cells / (kern_avg_ms * 1e-3) * 1e-12
         pk = peaks()
         hbm_gbs = 16.0 * nm * cells / (kern_avg_ms * 1e-3) * 1e-9
+        # what the kernel really moves: U and W(U) are both resident, i.e. read NV + NV and
+        # write NV + NV doubles per cell update with NV = 10 carried moments on the z-symmetric variant, 14 on the
+        # general one; the 5-moment kernel reads 5 and writes 5
+        nv = 5 if nm == 5 else (10 if s.fast_path_active else 14)
+        moved_model = 8.0 * (2 * nv if nm == 5 else 4 * nv) * cells
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             v, threads, secs = time_oracle(args.ref_n, args.kn, args.cpu_steps)
@@ -379,7 +388,8 @@ def run_gpu(args):
                          "flops_per_cell_update_oracle": fpc_oracle,
                          "flops_convention": "SURVEY.md 8(d): + - * / sqrt exp pow = 1 each, FMA = 2; a(P*), b(P*) of "
                                              "Eq 29c-d booked as the method's formulas, not as the table evaluation",
-                         "peak_source": "FP64 DFMA loop measured in this run (mm_measure_fp64_peak, libmm_bench.so)",
+                         "peak_source": "best of two register-resident FP64 DFMA loops measured in this run (multiplier in a "
+                                        "register / as an instruction immediate; mm_measure_fp64_peak, libmm_bench.so)",
                          "peak_sm_mhz": peak_mhz, "peak_nominal": nominal_tf,
                          "fp64_operand_rates": {"unit": "1e12 thread instructions/s, operands from distinct registers",
                                                 "dfma_three_registers": r_dfma3, "dmul": r_dmul, "dadd": r_dadd,
@@ -388,7 +398,13 @@ def run_gpu(args):
                                                         "(mm_measure_fp64_operand_rates; DESIGN.md 9.3)"},
                          "frac_of_nominal": achieved_tf / nominal_tf if nominal_tf else None,
                          "hbm_algorithmic_gbs": hbm_gbs, "hbm_peak_gbs": pk.get("hbm_gbs"),
-                         "hbm_frac": hbm_gbs / pk["hbm_gbs"] if pk.get("hbm_gbs") else None},
+                         "hbm_algorithmic_frac": hbm_gbs / pk["hbm_gbs"] if pk.get("hbm_gbs") else None,
+                         # bytes really moved per launch: the ncu capture where one exists, else the kernel's own count
+                         "hbm_moved_bytes_per_launch": traffic if traffic else moved_model,
+                         "hbm_moved_source": traffic_src if traffic else "2 x (NV + NV) doubles per cell update (U and W(U) resident)",
+                         "hbm_moved_gbs": (traffic if traffic else moved_model) / (kern_avg_ms * 1e-3) * 1e-9,
+                         "hbm_frac": ((traffic if traffic else moved_model) / (kern_avg_ms * 1e-3) * 1e-9 / pk["hbm_gbs"]
+                                      if pk.get("hbm_gbs") else None)},
             "cpu_baseline": cpu,
         }
         print(json.dumps(out), flush=True)

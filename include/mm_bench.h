@@ -13,8 +13,10 @@ extern "C" {
 #endif
 
 /* FP64 FMA peak of the current device, measured with a register-resident DFMA loop on `stream`
- * (cudaStream_t): 2 flop per FMA, best of `repeats` launches (16 independent chains per thread, 8 blocks
- * of 256 threads per SM).  This is the roofline denominator of this FP64-ALU-bound method;
+ * (cudaStream_t): 2 flop per FMA, best of `repeats` launches each of two forms of the loop -- multiplier and
+ * addend loop-invariant registers (2.17 scheduler cycles per DFMA measured), and the multiplier an instruction
+ * immediate (2.00 cycles, the pipe's issue rate) -- 16 independent chains per thread, 8 blocks of 256 threads
+ * per SM.  This is the roofline denominator of this FP64-ALU-bound method;
  * MEASURED_PEAKS.json has no FP64 entry.  If sm_mhz != NULL it receives the SM clock during the probe,
  * from the kernel's own clock64() / globaltimer readings (MHz). */
 int mm_measure_fp64_peak(void *stream, int repeats, double *tflops, double *sm_mhz);

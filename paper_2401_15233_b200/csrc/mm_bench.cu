@@ -12,6 +12,9 @@ namespace {
 // Register-resident DFMA loop: 16 independent chains per thread, 2 flop per FMA.  Thread 0 of every
 // block also reads the SM cycle counter and the nanosecond global timer around the loop, so the clock
 // the probe actually ran at is known (out[1 + 2 b], out[2 + 2 b] of block b).
+// IMM = true: the multiplier is the literal 1 - 2^-12, whose low word is zero, so it is encoded in the instruction
+// (DFMA R, R, imm, R): one register operand fewer to deliver per issue than with `a` in a register.
+template <bool IMM>
 __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a, double b)
 {
     double x[16];
@@ -22,7 +25,7 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, doubl
     if (threadIdx.x == 0) { c0 = clock64(); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(n0)); }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) x[k] = fma(x[k], a, b);
+        for (int k = 0; k < 16; ++k) x[k] = IMM ? fma(x[k], 0.999755859375, b) : fma(x[k], a, b);
     }
     if (threadIdx.x == 0) { c1 = clock64(); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(n1)); }
     double s = 0.0;
@@ -106,15 +109,16 @@ int mm_measure_fp64_peak(void* stream, int repeats, double* tflops, double* sm_m
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     double best = 0.0, mhz = 0.0;
     int rc = 0;
-    for (int r = 0; r < repeats + 1 && rc == 0; ++r) {            // first launch is the warm-up
+    for (int r = 0; r < 2 * (repeats + 1) && rc == 0; ++r) {      // both forms alternate; the first launch of each is the warm-up
         cudaEventRecord(e0, st);
-        k_dfma_peak<<<blocks, threads, 0, st>>>(d_out, iters, 0.999999, 1e-6);
+        if (r & 1) k_dfma_peak<true><<<blocks, threads, 0, st>>>(d_out, iters, 0.999999, 1e-6);
+        else k_dfma_peak<false><<<blocks, threads, 0, st>>>(d_out, iters, 0.999999, 1e-6);
         cudaEventRecord(e1, st);
         if (cudaEventSynchronize(e1) != cudaSuccess) { rc = -3; break; }
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
         const double tf = 2.0 * 16.0 * (double)iters * blocks * threads / (ms * 1e-3) * 1e-12;
-        if (r > 0 && tf > best) {
+        if (r > 1 && tf > best) {
             best = tf;
             if (cudaMemcpy(h_out, d_out, nout * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = -3; break; }
             double cyc = 0.0, ns = 0.0;

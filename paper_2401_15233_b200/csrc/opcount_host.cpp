@@ -53,11 +53,11 @@ inline cnt fmax(cnt a, double b) { return cnt(std::fmax(a.v, b)); }
 using namespace mm;
 
 // one limited half slope of cell c from its neighbours (computed once per cell and direction)
-template <int NM>
-static void half_slope(const Params& p, const cnt (&Wm)[NM], const cnt (&Wc)[NM], const cnt (&Wp)[NM],
-                       cnt (&h)[NM], bool zs)
+template <int NM, int LIM>
+static void half_slope_lim(const Params& p, const cnt (&Wm)[NM], const cnt (&Wc)[NM], const cnt (&Wp)[NM],
+                           cnt (&h)[NM], bool zs)
 {
-    PsiShared<1> pm;                                   // counted for minmod (p.limiter = 1 in main)
+    PsiShared<LIM> pm;                                 // the shared limiter value of this limiter kind
     for (int k = 0; k < NM; ++k) {
         if (NM == 14 && zs && z_odd(k)) continue;
         const cnt dm = Wc[k] - Wm[k], dp = Wp[k] - Wc[k];
@@ -74,7 +74,15 @@ static void half_slope(const Params& p, const cnt (&Wm)[NM], const cnt (&Wc)[NM]
     }
 }
 
-// interface M|C: face states from the two half slopes, two face evaluations, HLL
+template <int NM>
+static void half_slope(const Params& p, const cnt (&Wm)[NM], const cnt (&Wc)[NM], const cnt (&Wp)[NM],
+                       cnt (&h)[NM], bool zs)
+{
+    if (p.limiter == 2) half_slope_lim<NM, 2>(p, Wm, Wc, Wp, h, zs);
+    else half_slope_lim<NM, 1>(p, Wm, Wc, Wp, h, zs);
+}
+
+// interface M|C: face states from the two half slopes, two face evaluations, HLL or Rusanov (p.flux)
 template <int NM, class Z>
 static void interface(const Params& p, const cnt (&Wm)[NM], const cnt (&hm)[NM], const cnt (&Wc)[NM],
                       const cnt (&hc)[NM], cnt (&Fh)[NM])
@@ -88,6 +96,14 @@ static void interface(const Params& p, const cnt (&Wm)[NM], const cnt (&hm)[NM],
     cnt FL[NM], UL[NM], FR[NM], UR[NM], a, b, c, d;
     if constexpr (NM == 5) { eval_face5(p, WL, FL, UL, a, b); eval_face5(p, WR, FR, UR, c, d); }
     else { eval_face14<Z>(p, WL, FL, UL, a, b); eval_face14<Z>(p, WR, FR, UR, c, d); }
+    if (p.flux == 1) {                                 // Rusanov, as mm_tm14.cuh / mm_kernels.cuh write it
+        const cnt S = fmax(fmax(fabs(a), fabs(b)), fmax(fabs(c), fabs(d)));
+        for (int k = 0; k < NM; ++k) {
+            if (NM == 14 && zs && z_odd(k)) continue;
+            Fh[k] = 0.5 * (FL[k] + FR[k]) - 0.5 * S * (UR[k] - UL[k]);
+        }
+        return;
+    }
     const cnt SL = fmin(fmin(a, c), 0.0), SR = fmax(fmax(b, d), 0.0);
     const cnt inv = rcp(SR - SL), cL = SR * inv, cR = -SL * inv, cU = SL * cL;
     for (int k = 0; k < NM; ++k) {
@@ -149,9 +165,15 @@ int main()
     p.inv_tau_coef = 100.0; p.tau_model = 2; p.limiter = 1; p.flux = 0;
     // a(P*), b(P*) of Eq 29c-d are booked at the METHOD's operation count (pow, exp = 1 each: 10 per call);
     // the *_executed lines add what the kernel's table evaluation executes beyond that.
+    // keys: ..._{shared|per_variable}_limiter for minmod + HLL (the BASELINE configs); the other limiter / flux
+    // combinations carry the suffix _vanalbada and / or _rusanov (the paper's own jets: both)
+    for (int combo = 0; combo < 4; ++combo)
     for (int shared = 0; shared < 2; ++shared) {
         p.shared_limiter = shared;
-        const char* nm = shared ? "shared_limiter" : "per_variable_limiter";
+        p.limiter = (combo & 1) ? 2 : 1; p.flux = (combo & 2) ? 1 : 0;
+        char nm[96];
+        snprintf(nm, sizeof nm, "%s%s%s", shared ? "shared_limiter" : "per_variable_limiter",
+                 (combo & 1) ? "_vanalbada" : "", (combo & 2) ? "_rusanov" : "");
         long long n;
         g_ab_executed_flops = 0; n = one_cell<14, double>(p, 2);
         printf("kernel_flops_per_cell_update_14_%s %lld\n", nm, n);
