@@ -541,6 +541,27 @@ def test_dt_history_and_checkpoint_resume(mm, mmo):
     assert np.array_equal(s2.dt_history(60, 20), sg.dt_history(60, 20))
 
 
+@pytest.mark.parametrize("scheme", ["midpoint", "point_implicit"])
+@pytest.mark.parametrize("system", [14, 5])
+def test_checkpoint_resume_other_schemes(mm, scheme, system):
+    """include/mm.h promises that get_state + info / set_state + set_clock resume a run bit for bit, whatever the
+    scheme: the CFL rate of the restored state must come out of the same instructions that produced it in the
+    original run (midpoint: the second pass of a step; point-implicit source, L348)."""
+    opt = dict(time_scheme=wl.TIME_MIDPOINT) if scheme == "midpoint" else dict(source_scheme=wl.SRC_POINT_IMPLICIT)
+    prob = wl.crossed_jets(64, Kn=1.0, **opt) if system == 14 else wl.sod5(400, Kn=0.01, **opt)
+    sg = mm.Solver.from_problem(prob)
+    sg.step(40, 0.4)
+    U40, inf = sg.get_state(), sg.info()
+    sg.step(25, 0.4)
+    s2 = mm.Solver.from_problem(prob, load_state=False)
+    s2.set_state(U40); s2.set_clock(inf["t"], inf["steps"])
+    assert s2.cfl_dt(0.4) == sg.dt_history(40, 1)[0]            # the first dt after the checkpoint, to the bit
+    s2.step(25, 0.4)
+    assert np.array_equal(s2.dt_history(40, 25), sg.dt_history(40, 25))
+    assert np.array_equal(s2.get_state(), sg.get_state())
+    assert s2.info()["t"] == sg.info()["t"] and s2.info()["steps"] == 65
+
+
 # ------------------------------ SURVEY 8(f) item 4: batched 1-D 5-moment tubes (sigma_lim x Kn sweep)
 def _tube_oracles(mmo, nx, sigma_lims, Kns, **opt):
     out = []
