@@ -238,8 +238,12 @@ int set_state_impl(mm_solver* s, const double* src, int on_device, bool prim)
         // in the run a checkpoint was taken from, so that set_state + set_clock resumes that run bit for bit
         // (k_rate's inlined copy of the wave-speed code may be fused differently by the compiler; W(U) from
         // k_pack is bit-identical by construction, see cons2prim14).  The pass's copy of the state is dropped.
-        // ctrl->dt is 0 here (cleared above), so this is the very instantiation mm_step launches.
-        if ((rc = launch_pass(s, s->cur, s->cur ^ 1, nullptr, 1.0, 1))) return rc;
+        // ctrl->dt is 0 here (cleared above).  The pass must also be the INSTANTIATION whose tail produced the
+        // rate in the original run: launch_pass picks the EXT variant for the point-implicit source by itself;
+        // for the midpoint scheme the rate comes from a step's second pass, which has a base state, so this pass
+        // is given one too (the state itself: B - 0 * div F = B).
+        const double* base = s->time_scheme == MM_TIME_MIDPOINT ? s->U[s->cur] : nullptr;
+        if ((rc = launch_pass(s, s->cur, s->cur ^ 1, base, 1.0, 1))) return rc;
         s->slot ^= 1;
     }
     return MM_OK;
@@ -671,6 +675,7 @@ int mm_batch5_set_state_prim(mm_batch5* b, const double* W, int per_tube, int on
     }
     dim3 grid((b->nx + 127) / 128, b->ntubes);
     k_batch5_pack<<<grid, 128, 0, b->stream>>>(b->nx, b->ntubes, per_tube ? 1 : 0, src, b->U[b->cur]);
+    MM_CUDA(cudaGetLastError());
     MM_CUDA(cudaMemsetAsync(b->ctl, 0, (size_t)b->ntubes * sizeof(TubeCtl), b->stream));
     b->slot = 0;
     dim3 g2((b->nx + kNTB - 1) / kNTB, b->ntubes);
