@@ -4,7 +4,7 @@ developed (ill-conditioned) states that does not depend on how the scheme amplif
   * BASELINE configs[3] (2048^2 crossed jets): 100 steps at fixed dt on the FULL grid against the
     oracle, 1e-10 per moment (north_star; SURVEY.md section 8(d) "at 2048^2 once");
     configs[4] (4096^2): the same 100 steps on windows with a 2 x 100 + 1 cell margin, each window
-    scaled by its OWN per-moment maximum.
+    scaled by max(its own per-moment maximum, rho c^n) (reading R25; the fixed dt is reading R26).
   * Re-synchronised single steps: the oracle marches a developed state; before every step its state is
     handed to the GPU (mm_set_state), both take ONE step, every cell is compared.  Amplification across
     steps never enters, so the per-step bar is a property of one step's arithmetic.
@@ -83,7 +83,8 @@ def test_C5_4096_100_steps_windows(mm, mmo, fast):
     """configs[4] (4096^2, Kn 0.1): 100 fixed-dt steps; a cell depends on the 2-cell stencil per step,
     so the oracle recomputes windows of the same seeded state with a 201-cell margin to every cut edge
     (and none to the true left boundary, which the window keeps) and the inner cells are compared,
-    each window scaled by its own per-moment maximum.  Windows sit on the inflow bands, between them,
+    each window scaled by max(own per-moment maximum, rho c^n) (parity_util.window_errors, R25).
+    Windows sit on the inflow bands, between them,
     in the far field and across strip / row-chunk boundaries of the launch decomposition."""
     n, nsteps, margin, inner = 4096, 100, 201, 48
     prob = wl.crossed_jets(n, Kn=0.1, perturb=0.01)
