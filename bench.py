@@ -60,8 +60,8 @@ def flops_per_cell_update(shared_limiter: bool, zsym: bool, system: int = 14, li
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None where no capture of that configuration exists).
 NCU_TRAFFIC_BYTES = {
-    ("k_step14_tm<zsym>", 2048): (703.30e6 + 627.53e6, "profiles/r2d_k_step14_tm_zsym.md"),
-    ("k_step14_tm<general>", 2048): (971.75e6 + 897.79e6, "profiles/r2d_k_step14_tm_general.md"),
+    ("k_step14_tm<zsym>", 2048): (703.22e6 + 627.64e6, "profiles/r3_k_step14_tm_zsym.md"),
+    ("k_step14_tm<general>", 2048): (975.68e6 + 898.51e6, "profiles/r3_k_step14_tm_general.md"),
 }
 FP64_LANES_PER_SM = 64      # DFMA lanes of a B200 SM: nominal peak = SMs x 64 x 2 flop x SM clock
 
